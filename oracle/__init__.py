@@ -1,0 +1,163 @@
+"""CPU oracle for the BEST-2 transient-pipeline hot path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes wrapper around ``oracle/mdsm_oracle.c`` (plain C + OpenMP, written from
+/root/reference/PAPER.md: Eq. 1 at PAPER.md:93, brute-force dedispersion PAPER.md:96,
+channel/spectrum thresholding PAPER.md:79-81, n-sigma detection PAPER.md:110,116).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It imports nothing from
+``paper_1307_5700_b200`` and the CUDA library imports nothing from here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from ctypes import POINTER, c_double, c_int, c_int32, c_int64, c_uint8, c_uint32, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mdsm_oracle.c")
+_LIB = os.path.join(_HERE, "libmdsm_oracle.so")
+# -ffp-contract=off / no fast-math: every fp64 op is a single IEEE op in the order written.
+CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-Wall"]
+
+EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
+
+
+def build(force: bool = False) -> str:
+    """Compile the C oracle with gcc if the .so is missing or older than the source."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.run(["gcc", *CFLAGS, "-o", _LIB, _SRC, "-lm"], check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.orc_detect_f32.restype = c_int64
+        _lib.orc_detect_f64.restype = c_int64
+        _lib.orc_detect_u32.restype = c_int64
+        _lib.orc_num_threads.restype = c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_L().orc_num_threads())
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(c_void_p)
+
+
+def delay_table(nchans, f_top, foff, tsamp, dm_low, dm_step, ndms) -> np.ndarray:
+    """delay[d][c] per Eq. 1 with north_star's constant and rounding."""
+    out = np.empty((ndms, nchans), dtype=np.int32)
+    _L().orc_delay_table(c_int(nchans), c_double(f_top), c_double(foff), c_double(tsamp),
+                         c_double(dm_low), c_double(dm_step), c_int(ndms), _p(out))
+    return out
+
+
+def _check_in(x, dtype):
+    assert x.dtype == dtype and x.ndim == 3 and x.flags.c_contiguous, (x.dtype, x.shape)
+    return x.shape
+
+
+def dedisperse(x: np.ndarray, delay: np.ndarray, variant: str = "rows", want_abs: bool = True):
+    """out[b][d][t] = sum_c x[b][c][t + delay[d][c]], t < nsamps - max(delay).
+
+    f32 input -> (out fp64, absum fp64 or None); u8 input -> (out uint32, None).
+    variant: 'naive' (loops b,d,t,c) or 'rows' (loops b,d,c,t, OpenMP over (b,d)).
+    """
+    nb, nc, ns = x.shape
+    nd = delay.shape[0]
+    assert delay.shape == (nd, nc) and delay.dtype == np.int32 and delay.flags.c_contiguous
+    nso = ns - int(delay.max())
+    assert nso > 0
+    L = _L()
+    if x.dtype == np.float32:
+        _check_in(x, np.float32)
+        out = np.empty((nb, nd, nso), dtype=np.float64)
+        ab = np.empty((nb, nd, nso), dtype=np.float64) if want_abs else None
+        fn = L.orc_dedisperse_f32_naive if variant == "naive" else L.orc_dedisperse_f32_rows
+        fn(_p(x), c_int(nb), c_int(nc), c_int64(ns), _p(delay), c_int(nd), c_int64(nso), _p(out), _p(ab))
+        return out, ab
+    _check_in(x, np.uint8)
+    out = np.empty((nb, nd, nso), dtype=np.uint32)
+    fn = L.orc_dedisperse_u8_naive if variant == "naive" else L.orc_dedisperse_u8_rows
+    fn(_p(x), c_int(nb), c_int(nc), c_int64(ns), _p(delay), c_int(nd), c_int64(nso), _p(out))
+    return out, None
+
+
+def dedisperse_rows(x: np.ndarray, delay: np.ndarray, rows: np.ndarray, want_abs: bool = True):
+    """Same definition for selected series only; rows[i] = b*ndms + d."""
+    nb, nc, ns = x.shape
+    nd = delay.shape[0]
+    nso = ns - int(delay.max())
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    assert rows.min() >= 0 and rows.max() < nb * nd
+    L = _L()
+    if x.dtype == np.float32:
+        _check_in(x, np.float32)
+        out = np.empty((len(rows), nso), dtype=np.float64)
+        ab = np.empty((len(rows), nso), dtype=np.float64) if want_abs else None
+        L.orc_dedisperse_f32_sel(_p(x), c_int(nb), c_int(nc), c_int64(ns), _p(delay), c_int(nd), c_int64(nso),
+                                 _p(rows), c_int64(len(rows)), _p(out), _p(ab))
+        return out, ab
+    _check_in(x, np.uint8)
+    out = np.empty((len(rows), nso), dtype=np.uint32)
+    L.orc_dedisperse_u8_sel(_p(x), c_int(nb), c_int(nc), c_int64(ns), _p(delay), c_int(nd), c_int64(nso),
+                            _p(rows), c_int64(len(rows)), _p(out))
+    return out, None
+
+
+def rfi_clip(x: np.ndarray, window: int, k_chan: float, k_spec: float, debug: bool = False):
+    """In-place RFI clip of x[b][c][t] (readings B-i..B-viii).
+
+    Returns dict(chan_mask [nb][nc][ns/window] u8, spec_mask [nb][ns] u8) plus, with
+    debug=True, chan_mean/chan_sig/chan_thr/repl [nb][nc], spec_thr [nb][3]=(thr,mean,sig),
+    spec_sum [nb][ns].
+    """
+    nb, nc, ns = x.shape
+    assert x.flags.c_contiguous and x.flags.writeable
+    if window < 1 or ns % window:
+        raise ValueError("nsamps must be a multiple of window (reading B-viii)")
+    cm = np.empty((nb, nc, ns // window), dtype=np.uint8)
+    sm = np.empty((nb, ns), dtype=np.uint8)
+    dbg = {}
+    if debug:
+        dbg = dict(chan_mean=np.empty((nb, nc)), chan_sig=np.empty((nb, nc)), chan_thr=np.empty((nb, nc)),
+                   repl=np.empty((nb, nc)), spec_thr=np.empty((nb, 3)), spec_sum=np.empty((nb, ns)))
+    fn = {np.dtype(np.float32): _L().orc_rfi_clip_f32, np.dtype(np.uint8): _L().orc_rfi_clip_u8}[x.dtype]
+    rc = fn(_p(x), c_int(nb), c_int(nc), c_int64(ns), c_int(window), c_double(k_chan), c_double(k_spec),
+            _p(cm), _p(sm), _p(dbg.get("chan_mean")), _p(dbg.get("chan_sig")), _p(dbg.get("chan_thr")),
+            _p(dbg.get("repl")), _p(dbg.get("spec_thr")), _p(dbg.get("spec_sum")))
+    if rc != 0:
+        raise RuntimeError(f"orc_rfi_clip failed rc={rc}")
+    return dict(chan_mask=cm, spec_mask=sm, **dbg)
+
+
+def detect(series: np.ndarray, n_valid: int, snr_thresh: float, max_events: int | None = None):
+    """n-sigma detection on series[b][d][stride>=n_valid] (readings D-i..D-vii).
+
+    Returns (events structured array sorted by (beam, dm_idx, t), total_count, stats[nb][nd][2]=(mean,rms)).
+    """
+    assert series.ndim == 3 and series.flags.c_contiguous
+    nb, nd, stride = series.shape
+    assert 0 < n_valid <= stride
+    if max_events is None:
+        max_events = 1 << 22
+    ev = np.zeros(max_events, dtype=EVENT_DTYPE)
+    stats = np.empty((nb, nd, 2), dtype=np.float64)
+    fn = {np.dtype(np.float32): _L().orc_detect_f32, np.dtype(np.float64): _L().orc_detect_f64,
+          np.dtype(np.uint32): _L().orc_detect_u32}[series.dtype]
+    cnt = fn(_p(series), c_int64(nb * nd), c_int(nd), c_int64(stride), c_int64(n_valid),
+             c_double(snr_thresh), _p(ev), c_int64(max_events), _p(stats))
+    ev = ev[: min(cnt, max_events)]
+    ev = ev[np.lexsort((ev["t"], ev["dm_idx"], ev["beam"]))]
+    return ev, int(cnt), stats

@@ -1,0 +1,120 @@
+/*
+ * mdsm.h -- C ABI of libmdsm: the data-parallel hot path of the Medicina BEST-2
+ * multibeam transient pipeline (arXiv:1307.5700) on NVIDIA B200 (sm_100a).
+ *
+ *   RFI clip  ->  multibeam brute-force incoherent dedispersion  ->  n-sigma detection
+ *
+ * Citations are to /root/reference/PAPER.md (line numbers) and to the readings listed in
+ * DESIGN.md section 3.  All pointers named d_* are DEVICE pointers, h_* are HOST pointers.
+ * The caller owns every buffer it passes; the plan owns the delay table and its scratch.
+ * No function throws or exits; every int-returning call returns an MDSM_* status and leaves
+ * a message retrievable with mdsm_last_error() (thread-local) on failure.
+ *
+ * Layouts (dense, row-major, time fastest -- "beam/channel/time order"):
+ *   in  [nbeams][nchans][nsamps]   float (MDSM_F32) or uint8_t (MDSM_U8); channel 0 = f_top
+ *   out [nbeams][ndms][nsamps]     float (MDSM_F32) or uint32_t (MDSM_U8); row stride = nsamps,
+ *                                  only t < nsamps_out = nsamps - max_delay is written / valid
+ *                                  (overlap reading A3: Eq. 6)
+ * The device-pointer calls only enqueue work on `cuda_stream` (a cudaStream_t cast to void*;
+ * NULL = the legacy default stream); they never synchronise and never allocate.
+ * beam0/nb select a contiguous range of beams so that the host can drive beam groups on
+ * different streams ("parallelized across beams"); pointers always address the
+ * FULL [nbeams]... arrays, the call offsets them by beam0 itself.
+ */
+#ifndef MDSM_H
+#define MDSM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mdsm_plan mdsm_plan;                                 /* opaque */
+
+/* One detection: "(time, DM, intensity) triplets" per beam.  16 bytes. */
+typedef struct { int32_t beam, dm_idx, t; float snr; } mdsm_event;
+
+enum { MDSM_F32 = 0, MDSM_U8 = 1 };
+enum { MDSM_OK = 0, MDSM_EINVAL = -1, MDSM_ENOMEM = -2, MDSM_ECUDA = -3, MDSM_EOVERFLOW = 1 };
+
+/* Survey parameters of one buffer (PAPER.md:96 "observation and survey parameters", :190, :194).
+ *   f_top  centre frequency of channel 0 in MHz; channel c is at f_top + c*foff, foff < 0 (MHz)
+ *   tsamp  sampling time in s; nsamps = input samples per channel per call
+ *   DM trial d is dm_low + d*dm_step (pc cm^-3), d in [0, ndms)
+ * Builds, in fp64 on the host, delay(d,c) = floor(4.148808e3 * DM_d * (f_c^-2 - f_top^-2) / tsamp + 0.5)
+ * (Eq. 1; constant and rounding from BASELINE.json north_star), uploads it, and
+ * allocates the per-plan device scratch.  Uses the current CUDA device.
+ * Returns NULL on error (bad argument: nbeams,nchans,ndms < 1, foff >= 0, tsamp <= 0,
+ * dm_step < 0, dm_low < 0, nsamps <= max_delay; or allocation / CUDA failure). */
+mdsm_plan *mdsm_plan_create(int nbeams, int nchans, double f_top, double foff, double tsamp,
+                            int64_t nsamps, double dm_low, double dm_step, int ndms);
+void mdsm_plan_destroy(mdsm_plan *plan);                            /* NULL is a no-op */
+
+int64_t mdsm_plan_max_delay(const mdsm_plan *plan);                 /* delay(ndms-1, nchans-1) */
+int64_t mdsm_plan_nsamps_out(const mdsm_plan *plan);                /* nsamps - max_delay */
+/* Copies the delay table to h_delays[ndms][nchans] (host). */
+int mdsm_plan_get_delays(const mdsm_plan *plan, int32_t *h_delays);
+const char *mdsm_last_error(void);
+
+/* Plan options.  key "dedisp_kernel": 0 = auto, 1 = direct (global-load reference kernel),
+ * 2 = tiled (shared-memory staged, register-blocked).  Unknown key/value -> MDSM_EINVAL. */
+int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);
+/* Number of kernels this plan has launched since creation (all entry points). */
+int64_t mdsm_plan_launch_count(const mdsm_plan *plan);
+
+/* RFI thresholding of the input filterbank, in place (PAPER.md:79 channel thresholding,
+ * PAPER.md:81 spectrum thresholding; thresholds per north_star: k sigma above the mean).
+ * Per beam, over all nsamps samples, one-sided:
+ *  1. per channel c: mean_c, sig_c (population) and the replacement value repl_c
+ *     (u8: mean rounded half up; f32: (float)mean);
+ *  2. channel slices: non-overlapping chunks of `window` samples; a chunk is flagged when its
+ *     sum > window*mean_c + k_chan*sig_c*sqrt(window); flags are dilated by one chunk on either
+ *     side in time; flagged chunks are overwritten with repl_c;
+ *  3. whole spectra, on the data as modified by 2: s_t = sum_c x[c][t]; a spectrum is flagged
+ *     when s_t > mean_t(s) + k_spec*rms_t(s); flagged spectra are overwritten with repl_c.
+ * d_chan_mask [nbeams][nchans][nsamps/window] and d_spec_mask [nbeams][nsamps] receive 0/1
+ * (either may be NULL).  window >= 1 and nsamps % window == 0, else MDSM_EINVAL. */
+int mdsm_rfi_clip(mdsm_plan *plan, void *d_in, int dtype, int beam0, int nb,
+                  int window, double k_chan, double k_spec,
+                  uint8_t *d_chan_mask, uint8_t *d_spec_mask, void *cuda_stream);
+
+/* Brute-force incoherent dedispersion:
+ *   out[b][d][t] = sum_c in[b][c][t + delay(d,c)],   t in [0, nsamps_out)
+ * MDSM_F32: float in, float out (fp32 accumulation; |err| <= 1e-5 * sum_c|in| + 1e-6).
+ * MDSM_U8 : uint8 in, uint32 out, exact. */
+int mdsm_dedisperse(mdsm_plan *plan, const void *d_in, int dtype, int beam0, int nb,
+                    void *d_out, void *cuda_stream);
+
+/* n-sigma thresholding of every dedispersed series (normalisation PAPER.md:110).
+ * Per (beam, dm) over t < nsamps_out: mean and population rms of the series; an event
+ * (beam, dm_idx, t, snr) is appended for every sample with snr = (x - mean)/rms > snr_thresh
+ * (fp64 arithmetic; a series with rms == 0 emits nothing).  Events are appended in no
+ * particular order with warp-aggregated atomics.  *d_count (device, must be zeroed by the
+ * caller before the first beam group) is incremented by the number of events found; only
+ * events whose slot index < max_events are stored in d_events. */
+int mdsm_detect(mdsm_plan *plan, const void *d_out, int dtype, int beam0, int nb,
+                double snr_thresh, mdsm_event *d_events, int64_t max_events,
+                unsigned long long *d_count, void *cuda_stream);
+
+/* The whole chain from HOST buffers (per-beam threads copy their input to the GPU;
+ * north_star item 4: beam groups on separate CUDA streams with overlapped host-to-device copies).
+ * h_in [nbeams][nchans][nsamps] (pinned memory overlaps best); the clipped data is NOT copied back.
+ * clip is skipped when window == 0.  Events are copied to h_events (up to max_events) and
+ * *h_count receives the total found.  Device buffers are plan-owned and allocated on first use.
+ * Synchronises before returning.  Returns MDSM_EOVERFLOW if *h_count > max_events. */
+int mdsm_pipeline_host(mdsm_plan *plan, const void *h_in, int dtype,
+                       int window, double k_chan, double k_spec, double snr_thresh,
+                       mdsm_event *h_events, int64_t max_events, uint64_t *h_count,
+                       int nstreams);
+
+/* Register-only add-issue microbenchmark on all SMs of the current device (the measured
+ * denominator of the dedispersion roofline).
+ * kind 0: FADD, 1: FADD2 (add.f32x2, two results per lane-instruction), 2: integer add.
+ * *adds_per_s receives 32-bit add results per second.  Synchronises. */
+int mdsm_measure_add_peak(int kind, double *adds_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MDSM_H */

@@ -1,0 +1,185 @@
+"""ctypes binding of libmdsm.so -- argument marshalling only (see include/mdsm.h for semantics).
+
+Every function has the name and argument order of its C counterpart.  Device buffers are
+``torch`` CUDA tensors (or raw integer device pointers); streams are ``torch.cuda.Stream``
+objects, raw ``cudaStream_t`` integers, or None for torch's current stream.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import (POINTER, c_char_p, c_double, c_int, c_int32, c_int64, c_uint64, c_void_p)
+
+import numpy as np
+
+__all__ = [
+    "MDSM_F32", "MDSM_U8", "MDSM_OK", "MDSM_EINVAL", "MDSM_ENOMEM", "MDSM_ECUDA", "MDSM_EOVERFLOW",
+    "EVENT_DTYPE", "MdsmError", "lib_path",
+    "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
+    "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
+    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_pipeline_host", "mdsm_measure_add_peak",
+]
+
+MDSM_F32, MDSM_U8 = 0, 1
+MDSM_OK, MDSM_EINVAL, MDSM_ENOMEM, MDSM_ECUDA, MDSM_EOVERFLOW = 0, -1, -2, -3, 1
+EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libmdsm.so")
+
+
+class MdsmError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"mdsm status {status}: {msg}")
+        self.status = status
+
+
+def _load():
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(
+            f"{path} is missing: the CUDA extension has not been built "
+            "(run `python paper_1307_5700_b200/build.py`). There is no CPU fallback.")
+    L = ctypes.CDLL(path)
+    L.mdsm_plan_create.restype = c_void_p
+    L.mdsm_plan_create.argtypes = [c_int, c_int, c_double, c_double, c_double, c_int64, c_double, c_double, c_int]
+    L.mdsm_plan_destroy.restype = None
+    L.mdsm_plan_destroy.argtypes = [c_void_p]
+    L.mdsm_plan_max_delay.restype = c_int64
+    L.mdsm_plan_max_delay.argtypes = [c_void_p]
+    L.mdsm_plan_nsamps_out.restype = c_int64
+    L.mdsm_plan_nsamps_out.argtypes = [c_void_p]
+    L.mdsm_plan_launch_count.restype = c_int64
+    L.mdsm_plan_launch_count.argtypes = [c_void_p]
+    L.mdsm_plan_get_delays.restype = c_int
+    L.mdsm_plan_get_delays.argtypes = [c_void_p, c_void_p]
+    L.mdsm_last_error.restype = c_char_p
+    L.mdsm_last_error.argtypes = []
+    L.mdsm_plan_set_option.restype = c_int
+    L.mdsm_plan_set_option.argtypes = [c_void_p, c_char_p, c_int64]
+    L.mdsm_rfi_clip.restype = c_int
+    L.mdsm_rfi_clip.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_double, c_double, c_void_p,
+                                c_void_p, c_void_p]
+    L.mdsm_dedisperse.restype = c_int
+    L.mdsm_dedisperse.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
+    L.mdsm_detect.restype = c_int
+    L.mdsm_detect.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_double, c_void_p, c_int64, c_void_p, c_void_p]
+    L.mdsm_pipeline_host.restype = c_int
+    L.mdsm_pipeline_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, c_double, c_void_p,
+                                     c_int64, POINTER(c_uint64), c_int]
+    L.mdsm_measure_add_peak.restype = c_int
+    L.mdsm_measure_add_peak.argtypes = [c_int, POINTER(c_double)]
+    return L
+
+
+_L = _load()
+
+
+def _ptr(x) -> int | None:
+    """Device/host pointer of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _stream(s) -> int | None:
+    if s is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream
+
+
+def _dtype_of(x, dtype):
+    if dtype is not None:
+        return dtype
+    name = str(getattr(x, "dtype", ""))
+    if name.endswith("float32"):
+        return MDSM_F32
+    if name.endswith("uint8") or name.endswith("uint32") or name.endswith("int32"):
+        return MDSM_U8
+    raise TypeError(f"cannot infer mdsm dtype from {name!r}")
+
+
+def _check(rc: int, allow=(MDSM_OK,)):
+    if rc not in allow:
+        raise MdsmError(rc, mdsm_last_error())
+    return rc
+
+
+def mdsm_last_error() -> str:
+    return _L.mdsm_last_error().decode()
+
+
+def mdsm_plan_create(nbeams, nchans, f_top, foff, tsamp, nsamps, dm_low, dm_step, ndms) -> int:
+    h = _L.mdsm_plan_create(nbeams, nchans, f_top, foff, tsamp, nsamps, dm_low, dm_step, ndms)
+    if not h:
+        raise MdsmError(MDSM_EINVAL, mdsm_last_error())
+    return h
+
+
+def mdsm_plan_destroy(plan) -> None:
+    _L.mdsm_plan_destroy(plan)
+
+
+def mdsm_plan_max_delay(plan) -> int:
+    return _L.mdsm_plan_max_delay(plan)
+
+
+def mdsm_plan_nsamps_out(plan) -> int:
+    return _L.mdsm_plan_nsamps_out(plan)
+
+
+def mdsm_plan_launch_count(plan) -> int:
+    return _L.mdsm_plan_launch_count(plan)
+
+
+def mdsm_plan_get_delays(plan, ndms: int, nchans: int) -> np.ndarray:
+    out = np.empty((ndms, nchans), dtype=np.int32)
+    _check(_L.mdsm_plan_get_delays(plan, out.ctypes.data))
+    return out
+
+
+def mdsm_plan_set_option(plan, key: str, value: int) -> None:
+    _check(_L.mdsm_plan_set_option(plan, key.encode(), value))
+
+
+def mdsm_rfi_clip(plan, d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask=None, d_spec_mask=None,
+                  stream=None, dtype=None) -> None:
+    _check(_L.mdsm_rfi_clip(plan, _ptr(d_in), _dtype_of(d_in, dtype), beam0, nb, window, k_chan, k_spec,
+                            _ptr(d_chan_mask), _ptr(d_spec_mask), _stream(stream)))
+
+
+def mdsm_dedisperse(plan, d_in, beam0, nb, d_out, stream=None, dtype=None) -> None:
+    _check(_L.mdsm_dedisperse(plan, _ptr(d_in), _dtype_of(d_in, dtype), beam0, nb, _ptr(d_out), _stream(stream)))
+
+
+def mdsm_detect(plan, d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, stream=None, dtype=None) -> None:
+    _check(_L.mdsm_detect(plan, _ptr(d_out), _dtype_of(d_out, dtype), beam0, nb, snr_thresh, _ptr(d_events),
+                          max_events, _ptr(d_count), _stream(stream)))
+
+
+def mdsm_pipeline_host(plan, h_in, window, k_chan, k_spec, snr_thresh, h_events, max_events, nstreams=4,
+                       dtype=None):
+    """Returns (status, count); status is MDSM_OK or MDSM_EOVERFLOW."""
+    cnt = c_uint64(0)
+    rc = _L.mdsm_pipeline_host(plan, _ptr(h_in), _dtype_of(h_in, dtype), window, k_chan, k_spec, snr_thresh,
+                               _ptr(h_events), max_events, ctypes.byref(cnt), nstreams)
+    _check(rc, allow=(MDSM_OK, MDSM_EOVERFLOW))
+    return rc, int(cnt.value)
+
+
+def mdsm_measure_add_peak(kind: int) -> float:
+    v = c_double(0.0)
+    _check(_L.mdsm_measure_add_peak(kind, ctypes.byref(v)))
+    return float(v.value)

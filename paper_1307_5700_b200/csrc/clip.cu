@@ -1,0 +1,361 @@
+// RFI clip kernels (PAPER.md:79 channel thresholding, PAPER.md:81 spectrum thresholding;
+// thresholds per BASELINE.json north_star; readings B-i..B-ix in DESIGN.md section 3).
+//
+//   clip_channel_kernel   one CTA per (beam, channel) row: warp-shuffle reductions give the
+//                         chunk sums (kept in shared memory) and the row's S, Q; the same CTA
+//                         then thresholds, dilates and overwrites flagged chunks in place.
+//   clip_spec_sum_kernel  column sums s_t over channels of the modified data (coalesced rows,
+//                         channels split over the warps of a CTA, reduced through shared memory).
+//   clip_spec_stats_kernel  one CTA per beam: M1, M2 -> mean_s, sig_s, threshold.
+//   clip_spec_apply_kernel  flags spectra and overwrites flagged columns.
+//
+// Decisions are taken in fp64 with single IEEE operations in the oracle's order
+// (__dadd_rn/__dmul_rn/__ddiv_rn/__dsqrt_rn are never contracted to FMA).  With uint8 input
+// every sum is an exact integer, so masks are bit-reproducible; with float input the sums are
+// fp64 in a different (tree) order and may differ from the oracle only within the guard band B-ix.
+#include "mdsm_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+    static constexpr int V = 4;
+    using Vec = float4;
+    using Acc = double;  // S, Q, chunk sums
+    __device__ static void sums(const Vec &v, Acc &s, Acc &q)
+    {
+        double a = v.x, b = v.y, c = v.z, d = v.w;
+        s = (a + b) + (c + d);
+        q = (a * a + b * b) + (c * c + d * d);
+    }
+};
+template <> struct Elem<uint8_t> {
+    static constexpr int V = 16;
+    using Vec = uint4;
+    using Acc = unsigned long long;
+    __device__ static void sums(const Vec &v, Acc &s, Acc &q)
+    {
+        unsigned ss = 0, qq = 0;
+        const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                unsigned e = (w[i] >> (8 * k)) & 0xffu;
+                ss += e;
+                qq += e * e;
+            }
+        s = ss;
+        q = qq;
+    }
+};
+
+template <typename A> __device__ __forceinline__ A shfl_xor(A v, int m);
+template <> __device__ __forceinline__ double shfl_xor<double>(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+template <> __device__ __forceinline__ unsigned long long shfl_xor<unsigned long long>(unsigned long long v, int m)
+{
+    return __shfl_xor_sync(0xffffffffu, v, m);
+}
+
+template <typename A> __device__ __forceinline__ A warp_sum(A v)
+{
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) v += shfl_xor<A>(v, m);
+    return v;
+}
+
+template <typename A> __device__ A block_sum(A v, A *red /*[kWarps]*/)
+{
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    A t = 0;
+#pragma unroll
+    for (int i = 0; i < kWarps; ++i) t += red[i];
+    return t;
+}
+
+// mode 0: chunk = g lanes of one warp iteration (g power of two <= 32)
+// mode 1: chunk = g/32 warp iterations of one warp (g % 32 == 0)
+// mode 2: generic scalar path (any window, any alignment); chunk sums are recomputed from global
+template <typename T, int MODE>
+__global__ void __launch_bounds__(kThreads)
+clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps, int window, double k_chan,
+                    double *__restrict__ chan_stats, uint8_t *__restrict__ chan_mask)
+{
+    using E = Elem<T>;
+    using Acc = typename E::Acc;
+    constexpr int V = E::V;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const long long nchunk = nsamps / window;
+    // layout: [csum: nchunk doubles (MODE<2 only)] [raw: nchunk bytes]
+    double *csum = reinterpret_cast<double *>(smem_raw);
+    uint8_t *raw = smem_raw + (MODE < 2 ? (size_t)nchunk * sizeof(double) : 0);
+    __shared__ Acc red[kWarps];
+
+    const int c = blockIdx.x;
+    const int b = beam0 + blockIdx.y;
+    T *row = in + ((size_t)b * nchans + c) * (size_t)nsamps;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    Acc S = 0, Q = 0;
+    if (MODE == 0) {
+        const int g = window / V;
+        const long long nvec = nsamps / V;
+        const typename E::Vec *vrow = reinterpret_cast<const typename E::Vec *>(row);
+        for (long long base = 0; base < nvec; base += kThreads) {
+            const long long i = base + tid;
+            Acc s = 0, q = 0;
+            if (i < nvec) E::sums(vrow[i], s, q);
+            S += s;
+            Q += q;
+            for (int m = 1; m < g; m <<= 1) s += shfl_xor<Acc>(s, m);
+            if (i < nvec && (lane & (g - 1)) == 0) csum[i / g] = (double)s;
+        }
+    } else if (MODE == 1) {
+        const int g = window / V;
+        const typename E::Vec *vrow = reinterpret_cast<const typename E::Vec *>(row);
+        for (long long j = warp; j < nchunk; j += kWarps) {
+            Acc s = 0, q = 0;
+            for (int k = lane; k < g; k += 32) {
+                Acc s1, q1;
+                E::sums(vrow[j * g + k], s1, q1);
+                s += s1;
+                q += q1;
+            }
+            S += s;
+            Q += q;
+            s = warp_sum(s);
+            if (lane == 0) csum[j] = (double)s;
+        }
+    } else {
+        for (long long t = tid; t < nsamps; t += kThreads) {
+            Acc v = (Acc)row[t];
+            S += v;
+            Q += v * v;
+        }
+    }
+    S = block_sum(S, red);
+    Q = block_sum(Q, red);
+
+    // B1: per-channel statistics, single IEEE ops in the oracle's order
+    const double dN = (double)nsamps;
+    const double mean = __ddiv_rn((double)S, dN);
+    double var = __dsub_rn(__ddiv_rn((double)Q, dN), __dmul_rn(mean, mean));
+    if (var < 0.0) var = 0.0;
+    const double sig = __dsqrt_rn(var);
+    const double thr = __dadd_rn(__dmul_rn((double)window, mean), __dmul_rn(__dmul_rn(k_chan, sig), __dsqrt_rn((double)window)));
+    T repl;
+    if (sizeof(T) == 1)
+        repl = (T)(((unsigned long long)S + (unsigned long long)(nsamps / 2)) / (unsigned long long)nsamps);
+    else
+        repl = (T)mean;
+    if (tid == 0) {
+        double *st = chan_stats + ((size_t)b * nchans + c) * 4;
+        st[0] = mean; st[1] = sig; st[2] = thr; st[3] = (double)repl;
+    }
+
+    // B2: raw flags
+    for (long long j = tid; j < nchunk; j += kThreads) {
+        double C;
+        if (MODE < 2) {
+            C = csum[j];
+        } else {
+            Acc s = 0;
+            for (int k = 0; k < window; ++k) s += (Acc)row[j * window + k];
+            C = (double)s;
+        }
+        raw[j] = (C > thr) ? 1 : 0;
+    }
+    __syncthreads();
+    // dilation by one chunk in time, mask output, in-place replacement
+    uint8_t *mrow = chan_mask ? chan_mask + ((size_t)b * nchans + c) * (size_t)nchunk : nullptr;
+    for (long long j = tid; j < nchunk; j += kThreads) {
+        uint8_t m = raw[j];
+        if (j > 0) m |= raw[j - 1];
+        if (j + 1 < nchunk) m |= raw[j + 1];
+        if (mrow) mrow[j] = m;
+        if (m) {
+            T *x = row + j * window;
+            for (int k = 0; k < window; ++k) x[k] = repl;
+        }
+    }
+}
+
+// s_t = sum_c x[c][t] on the data as modified by the channel stage (B3, first half).
+// CTA = 8 warps; covers 32*V consecutive samples; warp w adds channels c = w, w+8, ...
+template <typename T, bool VEC>
+__global__ void __launch_bounds__(kThreads)
+clip_spec_sum_kernel(const T *__restrict__ in, int beam0, int nchans, long long nsamps, double *__restrict__ spec_sum)
+{
+    using E = Elem<T>;
+    constexpr int V = VEC ? E::V : 1;
+    using Acc = typename E::Acc;
+    __shared__ Acc part[kWarps][32 * V + 1];
+    const int b = beam0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long t0 = ((long long)blockIdx.x * 32 + lane) * V;
+    const T *base = in + (size_t)b * nchans * (size_t)nsamps;
+    Acc acc[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) acc[k] = 0;
+    if (t0 < nsamps) {
+        if (VEC) {
+#pragma unroll 4
+            for (int c = warp; c < nchans; c += kWarps) {
+                const typename E::Vec v = *reinterpret_cast<const typename E::Vec *>(base + (size_t)c * nsamps + t0);
+                if (sizeof(T) == 4) {
+                    const float *f = reinterpret_cast<const float *>(&v);
+#pragma unroll
+                    for (int k = 0; k < V; ++k) acc[k] += (Acc)f[k];
+                } else {
+                    const unsigned *w = reinterpret_cast<const unsigned *>(&v);
+#pragma unroll
+                    for (int k = 0; k < V; ++k) acc[k] += (Acc)((w[k >> 2] >> (8 * (k & 3))) & 0xffu);
+                }
+            }
+        } else {
+            for (int c = warp; c < nchans; c += kWarps) acc[0] += (Acc)base[(size_t)c * nsamps + t0];
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < V; ++k) part[warp][lane * V + k] = acc[k];
+    __syncthreads();
+    for (int i = threadIdx.x; i < 32 * V; i += kThreads) {
+        Acc s = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) s += part[w][i];
+        const long long t = (long long)blockIdx.x * 32 * V + i;
+        if (t < nsamps) spec_sum[(size_t)b * nsamps + t] = (double)s;
+    }
+}
+
+// One CTA per beam: M1 = sum s_t, M2 = sum s_t^2 -> spec_stats[b] = {thr, mean, sig}
+template <bool IS_INT>
+__global__ void __launch_bounds__(1024)
+clip_spec_stats_kernel(const double *__restrict__ spec_sum, int beam0, long long nsamps, double k_spec,
+                       double *__restrict__ spec_stats)
+{
+    const int b = beam0 + blockIdx.x;
+    const double *s = spec_sum + (size_t)b * nsamps;
+    __shared__ double rd[32][2];
+    __shared__ unsigned long long ru[32][2];
+    double m1 = 0.0, m2 = 0.0;
+    unsigned long long u1 = 0, u2 = 0;
+    for (long long t = threadIdx.x; t < nsamps; t += blockDim.x) {
+        const double v = s[t];
+        if (IS_INT) {
+            const unsigned long long u = (unsigned long long)v;
+            u1 += u;
+            u2 += u * u;
+        } else {
+            m1 += v;
+            m2 += v * v;
+        }
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (IS_INT) {
+        u1 = warp_sum(u1); u2 = warp_sum(u2);
+        if (lane == 0) { ru[warp][0] = u1; ru[warp][1] = u2; }
+    } else {
+        m1 = warp_sum(m1); m2 = warp_sum(m2);
+        if (lane == 0) { rd[warp][0] = m1; rd[warp][1] = m2; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double M1, M2;
+        if (IS_INT) {
+            unsigned long long a = 0, q = 0;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { a += ru[i][0]; q += ru[i][1]; }
+            M1 = (double)a; M2 = (double)q;
+        } else {
+            M1 = 0.0; M2 = 0.0;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { M1 += rd[i][0]; M2 += rd[i][1]; }
+        }
+        const double dN = (double)nsamps;
+        const double mean = __ddiv_rn(M1, dN);
+        double var = __dsub_rn(__ddiv_rn(M2, dN), __dmul_rn(mean, mean));
+        if (var < 0.0) var = 0.0;
+        const double sig = __dsqrt_rn(var);
+        spec_stats[4 * b + 0] = __dadd_rn(mean, __dmul_rn(k_spec, sig));
+        spec_stats[4 * b + 1] = mean;
+        spec_stats[4 * b + 2] = sig;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+clip_spec_apply_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps, const double *__restrict__ spec_sum,
+                       const double *__restrict__ spec_stats, const double *__restrict__ chan_stats,
+                       uint8_t *__restrict__ spec_mask)
+{
+    const int b = beam0 + blockIdx.y;
+    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (t >= nsamps) return;
+    const bool flag = spec_sum[(size_t)b * nsamps + t] > spec_stats[4 * b];
+    if (spec_mask) spec_mask[(size_t)b * nsamps + t] = flag ? 1 : 0;
+    if (flag) {
+        T *col = in + (size_t)b * nchans * (size_t)nsamps + t;
+        const double *st = chan_stats + (size_t)b * nchans * 4;
+        for (int c = 0; c < nchans; ++c) col[(size_t)c * nsamps] = (T)st[4 * c + 3];
+    }
+}
+
+template <typename T>
+int launch_clip_t(mdsm_plan *p, T *in, int beam0, int nb, int window, double k_chan, double k_spec,
+                  uint8_t *chan_mask, uint8_t *spec_mask, cudaStream_t st)
+{
+    constexpr int V = Elem<T>::V;
+    const long long nsamps = p->nsamps;
+    const long long nchunk = nsamps / window;
+    const bool aligned = ((uintptr_t)in % 16 == 0) && (nsamps % V == 0);
+    int mode = 2;
+    if (aligned && window % V == 0) {
+        const int g = window / V;
+        if (g <= 32 && (g & (g - 1)) == 0) mode = 0;
+        else if (g % 32 == 0) mode = 1;
+    }
+    size_t smem = (size_t)nchunk + (mode < 2 ? (size_t)nchunk * sizeof(double) : 0);
+    if (mode < 2 && smem > 200 * 1024) { mode = 2; smem = (size_t)nchunk; }
+    MDSM_REQUIRE(smem <= 200 * 1024, "nsamps/window = %lld chunks per channel exceeds the shared-memory flag buffer", nchunk);
+    dim3 grid1(p->nchans, nb);
+    auto k0 = clip_channel_kernel<T, 0>;
+    auto k1 = clip_channel_kernel<T, 1>;
+    auto k2 = clip_channel_kernel<T, 2>;
+    auto kern = mode == 0 ? k0 : (mode == 1 ? k1 : k2);
+    if (smem > 48 * 1024) MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid1, kThreads, smem, st>>>(in, beam0, p->nchans, nsamps, window, k_chan, p->d_chan_stats, chan_mask);
+    MDSM_CUDA_TRY(cudaGetLastError());
+
+    double *spec_stats = p->d_spec_part;  // [nbeams][4]
+    if (aligned) {
+        dim3 grid2((unsigned)((nsamps + 32 * V - 1) / (32 * V)), nb);
+        clip_spec_sum_kernel<T, true><<<grid2, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum);
+    } else {
+        dim3 grid2((unsigned)((nsamps + 31) / 32), nb);
+        clip_spec_sum_kernel<T, false><<<grid2, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum);
+    }
+    MDSM_CUDA_TRY(cudaGetLastError());
+    clip_spec_stats_kernel<sizeof(T) == 1><<<nb, 1024, 0, st>>>(p->d_spec_sum, beam0, nsamps, k_spec, spec_stats);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    dim3 grid4((unsigned)((nsamps + kThreads - 1) / kThreads), nb);
+    clip_spec_apply_kernel<T><<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats,
+                                                          p->d_chan_stats, spec_mask);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    p->launches += 4;
+    return MDSM_OK;
+}
+
+}  // namespace
+
+int mdsm_launch_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int nb, int window, double k_chan,
+                     double k_spec, uint8_t *d_chan_mask, uint8_t *d_spec_mask, cudaStream_t st)
+{
+    if (dtype == MDSM_F32)
+        return launch_clip_t<float>(p, (float *)d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask, d_spec_mask, st);
+    return launch_clip_t<uint8_t>(p, (uint8_t *)d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask, d_spec_mask, st);
+}

@@ -1,0 +1,163 @@
+// Detection kernels (PAPER.md:116 n-sigma thresholding; normalisation by the series' own
+// mean / standard deviation; readings D-i..D-vii in DESIGN.md section 3).
+//
+//   series_stats_kernel  one CTA per (beam, dm) series: S, Q over t < nsamps_out by warp-shuffle
+//                        reduction (uint64 exact for uint32 series, fp64 for float series),
+//                        then mean / rms with single IEEE fp64 ops in the oracle's order.
+//   threshold_emit_kernel  every sample: snr = ((double)x - mean)/rms > thr ?  Candidates are
+//                        pre-filtered with one fp64 subtract-compare; events are appended with
+//                        warp-aggregated atomics (one atomicAdd per warp per vote).
+#include "mdsm_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+
+template <typename A> __device__ __forceinline__ A wsum(A v)
+{
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+    return v;
+}
+
+template <typename T> __device__ __forceinline__ T as_elem(unsigned w);
+template <> __device__ __forceinline__ float as_elem<float>(unsigned w) { return __uint_as_float(w); }
+template <> __device__ __forceinline__ uint32_t as_elem<uint32_t>(unsigned w) { return w; }
+
+template <typename T> struct SAcc;
+template <> struct SAcc<float> { using type = double; };
+template <> struct SAcc<uint32_t> { using type = unsigned long long; };
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+series_stats_kernel(const T *__restrict__ out, int beam0, int ndms, long long nsamps, long long n,
+                    double *__restrict__ stats)
+{
+    using A = typename SAcc<T>::type;
+    const int d = blockIdx.x, b = beam0 + blockIdx.y;
+    const T *x = out + ((size_t)b * ndms + d) * (size_t)nsamps;
+    A S = 0, Q = 0;
+    const bool vec = ((uintptr_t)x % 16 == 0);
+    if (vec) {
+        const long long n4 = n / 4;
+        const uint4 *xv = reinterpret_cast<const uint4 *>(x);
+        for (long long i = threadIdx.x; i < n4; i += kThreads) {
+            const uint4 v = xv[i];
+            const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const A e = (A)as_elem<T>(w[k]);
+                S += e;
+                Q += e * e;
+            }
+        }
+        for (long long i = n4 * 4 + threadIdx.x; i < n; i += kThreads) {
+            A e = (A)x[i];
+            S += e;
+            Q += e * e;
+        }
+    } else {
+        for (long long i = threadIdx.x; i < n; i += kThreads) {
+            A e = (A)x[i];
+            S += e;
+            Q += e * e;
+        }
+    }
+    __shared__ A red[2][kThreads / 32];
+    S = wsum(S);
+    Q = wsum(Q);
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = S; red[1][threadIdx.x >> 5] = Q; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        A s = 0, q = 0;
+        for (int i = 0; i < kThreads / 32; ++i) { s += red[0][i]; q += red[1][i]; }
+        const double dn = (double)n;
+        const double mean = __ddiv_rn((double)s, dn);
+        double var = __dsub_rn(__ddiv_rn((double)q, dn), __dmul_rn(mean, mean));
+        if (var < 0.0) var = 0.0;
+        double *o = stats + ((size_t)b * ndms + d) * 2;
+        o[0] = mean;
+        o[1] = __dsqrt_rn(var);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+threshold_emit_kernel(const T *__restrict__ out, int beam0, int ndms, long long nsamps, long long n,
+                      const double *__restrict__ stats, double thr, mdsm_event *__restrict__ events,
+                      long long max_events, unsigned long long *__restrict__ count)
+{
+    const int d = blockIdx.y, b = beam0 + blockIdx.z;
+    const double mean = stats[((size_t)b * ndms + d) * 2];
+    const double rms = stats[((size_t)b * ndms + d) * 2 + 1];
+    if (rms == 0.0) return;                          // whole CTA: uniform
+    // snr > thr  =>  x - mean > thr*rms*(1 - 2^-40): cheap conservative pre-filter (thr*rms >= 0);
+    // for negative thresholds every sample is a candidate.
+    const double cut = thr > 0.0 ? thr * rms * (1.0 - 9.094947017729282e-13) : -1.7976931348623157e308;
+    const T *x = out + ((size_t)b * ndms + d) * (size_t)nsamps;
+    const long long t0 = ((long long)blockIdx.x * kThreads + threadIdx.x) * 4;
+    T v[4];
+    if (t0 + 3 < n && ((uintptr_t)x % 16 == 0)) {
+        const uint4 u = *reinterpret_cast<const uint4 *>(x + t0);
+        const unsigned w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = as_elem<T>(w[k]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (t0 + k < n) ? x[t0 + k] : (T)0;
+    }
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        bool hit = false;
+        double snr = 0.0;
+        if (t0 + k < n) {
+            const double dv = __dsub_rn((double)v[k], mean);
+            if (dv > cut) {
+                snr = __ddiv_rn(dv, rms);
+                hit = snr > thr;
+            }
+        }
+        const unsigned ballot = __ballot_sync(0xffffffffu, hit);
+        if (ballot) {
+            unsigned long long base = 0;
+            const int leader = __ffs(ballot) - 1;
+            if (lane == leader) base = atomicAdd(count, (unsigned long long)__popc(ballot));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (hit) {
+                const unsigned long long slot = base + __popc(ballot & ((1u << lane) - 1));
+                if (slot < (unsigned long long)max_events) {
+                    mdsm_event e;
+                    e.beam = b; e.dm_idx = d; e.t = (int32_t)(t0 + k); e.snr = (float)snr;
+                    events[slot] = e;
+                }
+            }
+        }
+    }
+}
+
+template <typename T>
+int launch_detect_t(mdsm_plan *p, const T *out, int beam0, int nb, double thr, mdsm_event *ev, long long max_events,
+                    unsigned long long *count, cudaStream_t st)
+{
+    MDSM_REQUIRE(p->ndms <= 65535 && nb <= 65535, "ndms and nb must be <= 65535");
+    dim3 g1(p->ndms, nb);
+    series_stats_kernel<T><<<g1, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    dim3 g2((unsigned)((p->nsamps_out + kThreads * 4 - 1) / (kThreads * 4)), p->ndms, nb);
+    threshold_emit_kernel<T><<<g2, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats,
+                                                      thr, ev, max_events, count);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    p->launches += 2;
+    return MDSM_OK;
+}
+
+}  // namespace
+
+int mdsm_launch_detect(mdsm_plan *p, const void *d_out, int dtype, int beam0, int nb, double snr_thresh,
+                       mdsm_event *d_events, int64_t max_events, unsigned long long *d_count, cudaStream_t st)
+{
+    if (dtype == MDSM_F32)
+        return launch_detect_t<float>(p, (const float *)d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, st);
+    return launch_detect_t<uint32_t>(p, (const uint32_t *)d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, st);
+}

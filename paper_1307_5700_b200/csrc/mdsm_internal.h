@@ -35,7 +35,7 @@ struct TiledTables {
     int row_words = 0;                            // staged words per channel row
     int max_off = 0;                              // largest per-DM register offset
     int32_t *d_row_start = nullptr;               // [n_dm_blocks][nchans]   first staged sample - tile_t0
-    uint32_t *d_warp_tab = nullptr;               // [n_dm_blocks*warps][nchans] packed window base + per-DM offsets
+    void *d_warp_tab = nullptr;                   // [n_dm_blocks][nslab][warps][CS] packed window base + per-DM offsets
     int32_t *d_sigma = nullptr;                   // [n_dm_blocks*dm_block]  output time shear per DM
     int sigma_max = 0;
     bool ok = false;

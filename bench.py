@@ -135,6 +135,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="dedisp_kernel option: 0 auto, 1 direct, 2 tiled")
+    ap.add_argument("--geom", type=int, default=-1, help="tiled_geom_<dtype> option (compiled tile geometry); -1 = plan default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--nstreams", type=int, default=4)
@@ -169,6 +170,8 @@ def main():
     work = torch.empty_like(pristine)
     plan = m.mdsm_plan_create(*cfg.plan_args())
     m.mdsm_plan_set_option(plan, "dedisp_kernel", args.kernel)
+    if args.geom >= 0:
+        m.mdsm_plan_set_option(plan, "tiled_geom_" + cfg.dtype, args.geom)
     nso = m.mdsm_plan_nsamps_out(plan)
     out = torch.empty((cfg.nbeams, cfg.ndms, cfg.nsamps), dtype=torch.float32 if cfg.dtype == "f32" else torch.int32,
                       device="cuda")
@@ -267,7 +270,7 @@ def main():
         "config": {"workload": cfg.name, "nbeams_per_gpu": cfg.nbeams, "nchans": cfg.nchans, "nsamps": cfg.nsamps,
                    "ndms": cfg.ndms, "chain": "rfi_clip+dedisperse+detect", "snr_thresh": cfg.snr_thresh,
                    "l2": "input restored from a pristine 2.1 GB copy before every step (larger than L2)",
-                   "dedisp_kernel": args.kernel},
+                   "dedisp_kernel": args.kernel, "tiled_geom": args.geom},
         "realtime_beams_640dm": cfg.nbeams * world * nso * cfg.tsamp / (ms_per_step * 1e-3),
         "stage_ms": {"rfi_clip": statistics.mean(clip_ms), "dedisperse": statistics.mean(dd_ms), "detect": statistics.mean(det_ms)},
         "dedisperse_only": {"value": units_per_step / world / dd, "unit": "DM-trial samples/s"},

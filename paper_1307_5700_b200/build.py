@@ -28,7 +28,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    subprocess.run([sys.executable, os.path.join(CSRC, "gen_vadd.py"), os.path.join(CSRC, "vadd_gen.h")], check=True)
+    subprocess.run([sys.executable, os.path.join(CSRC, "gen_chain.py"), os.path.join(CSRC, "chain_gen.h")], check=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, *NVCC_FLAGS, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:

@@ -10,8 +10,9 @@
 // from shared memory with conflict-free 128-bit loads (T/4 is odd) and adds it, at D different
 // register offsets, into its D accumulator rows -- every shared-memory word feeds ~3 adds, which is
 // what lifts the kernel off the 32 words/clk/SM shared-memory ceiling (25 % of the add peak).
-// The offsets are warp-uniform; each is applied with one indirect branch into a straight-line
-// block of adds (vadd_gen.h).
+// The offsets are warp-uniform; they select straight-line add blocks through a threaded chain of
+// indirect branches (chain_gen.h).  fp32 accumulators and window are packed f32x2 register pairs so
+// that an even offset costs T/2 issue slots (FADD2) -- the FMA pipe, not the issue port, is the limit.
 // The time axis is SHEARED: DM d of a block owns outputs [tile_t0 - sigma_d, tile_t0 - sigma_d + 32T)
 // with sigma_d ~ half the band-edge delay slope, which halves the spread of the D windows (and of
 // the staged rows) compared with an unsheared tile.
@@ -22,8 +23,8 @@
 #include <cmath>
 #include <vector>
 
+#include "chain_gen.h"
 #include "mdsm_internal.h"
-#include "vadd_gen.h"
 
 namespace {
 
@@ -61,10 +62,96 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
+__device__ __forceinline__ void lds128(unsigned long long &a, unsigned long long &b, uint32_t addr)
+{
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
+}
 
-// ------------------------------------------------------------------ kernel
-// warp_tab entry (64 bit): bits 0..15 window start (in float4 units, relative to the staged row),
-// bits 16..19 number of float4 chunks to load beyond T/4 (adaptive window), byte 3+j: offset of DM j.
+// predicated form: one SASS instruction, no branch (the registers keep stale data when pred is false)
+__device__ __forceinline__ void lds128_if(unsigned long long &a, unsigned long long &b, uint32_t addr, bool pred)
+{
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q ld.shared.v2.b64 {%0, %1}, [%2]; }" : "=l"(a), "=l"(b) : "r"(addr), "r"((unsigned)pred));
+}
+
+// Stores v[0..T) to orow[ts .. ts+T), clipped to [0, n).  Rows are 16-byte aligned; ts is not (the
+// shear is a whole number of samples), so the head up to the next multiple of 4 goes out as scalars and
+// the rest as 128-bit stores.  The head length is warp-uniform: one switch, static register indexing.
+template <int T, int H, typename V>
+__device__ __forceinline__ void store_row_h(V *orow, long long ts, long long n, const V (&v)[T])
+{
+#pragma unroll
+    for (int i = 0; i < H; ++i)
+        if (ts + i >= 0 && ts + i < n) orow[ts + i] = v[i];
+#pragma unroll
+    for (int i = H; i + 3 < T; i += 4) {
+        const long long t = ts + i;
+        if (t >= 0 && t + 3 < n) {
+            uint4 q;
+            q.x = reinterpret_cast<const uint32_t &>(v[i]); q.y = reinterpret_cast<const uint32_t &>(v[i + 1]);
+            q.z = reinterpret_cast<const uint32_t &>(v[i + 2]); q.w = reinterpret_cast<const uint32_t &>(v[i + 3]);
+            *reinterpret_cast<uint4 *>(orow + t) = q;
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k >= 0 && t + k < n) orow[t + k] = v[i + k];
+        }
+    }
+#pragma unroll
+    for (int i = H + (T - H) / 4 * 4; i < T; ++i)
+        if (ts + i >= 0 && ts + i < n) orow[ts + i] = v[i];
+}
+template <int T, typename V>
+__device__ __forceinline__ void store_row(V *orow, long long ts, long long n, const V (&v)[T])
+{
+    static_assert(sizeof(V) == 4, "32-bit outputs");
+    switch ((int)((4 - (ts & 3)) & 3)) {
+        case 0: store_row_h<T, 0>(orow, ts, n, v); break;
+        case 1: store_row_h<T, 1>(orow, ts, n, v); break;
+        case 2: store_row_h<T, 2>(orow, ts, n, v); break;
+        default: store_row_h<T, 3>(orow, ts, n, v); break;
+    }
+}
+
+// ------------------------------------------------------------------ producer (shared by the dtypes)
+// Lane r < CS copies row r of every slab, lane CS copies the slab's slice of the warp table.
+template <typename TIn, int NW, int CS>
+__device__ __forceinline__ void producer_loop(const TIn *__restrict__ beam_in, const int32_t *__restrict__ rs,
+                                              const unsigned long long *__restrict__ wtab, unsigned char *rows,
+                                              unsigned long long *tabs, uint64_t *full, uint64_t *empty, long long tile_t0,
+                                              int nchans, int nslab, long long nsamps, int row_elems, int stages, int lane)
+{
+    int st = 0;
+    uint32_t ph = 1;            // parity of the empty-barrier phase to wait for (first lap: no wait)
+    for (int slab = 0; slab < nslab; ++slab, ++st) {
+        if (st == stages) { st = 0; ph ^= 1; }
+        if (slab >= stages) mbar_wait(&empty[st], ph);
+        if (lane < CS) {
+            const int c = slab * CS + lane;
+            uint32_t bytes = 0;
+            long long lo = 0, g0 = 0;
+            if (c < nchans) {
+                g0 = tile_t0 + rs[c];
+                lo = g0 < 0 ? 0 : g0;
+                long long hi = g0 + row_elems;
+                if (hi > nsamps) hi = nsamps;
+                if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(TIn));
+            }
+            mbar_arrive_expect_tx(&full[st], bytes);
+            if (bytes)
+                bulk_g2s(rows + (((size_t)st * CS + lane) * row_elems + (lo - g0)) * sizeof(TIn),
+                         beam_in + (size_t)c * nsamps + lo, bytes, &full[st]);
+        } else if (lane == CS) {
+            const uint32_t bytes = NW * CS * sizeof(unsigned long long);
+            mbar_arrive_expect_tx(&full[st], bytes);
+            bulk_g2s(tabs + (size_t)st * NW * CS, wtab + (size_t)slab * NW * CS, bytes, &full[st]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ fp32 kernel
+// warp_tab entry (64 bit): bits 0..15 window start in 16-byte units relative to the stage base (row r
+// included), bits 16..19 number of 16-byte chunks to load beyond T/4 (adaptive window), byte 3+j:
+// register offset of DM j.
 template <int D, int T, int NW, int CS, int NOFF>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ out, const int32_t *__restrict__ row_start,
@@ -74,11 +161,11 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
 {
     static_assert(T % 4 == 0 && (T / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
     static_assert(D <= 5, "table entry holds at most 5 offsets");
-    constexpr int W = T + NOFF;
+    using Chain = ChainF32<D, T, NOFF>;
+    constexpr int W2 = Chain::W2;           // window length in f32x2 pairs
     constexpr int DB = D * NW;
     extern __shared__ __align__(128) unsigned char smem[];
     const size_t stage_bytes = (size_t)CS * row_words * sizeof(float);
-    float *rows = reinterpret_cast<float *>(smem);
     unsigned long long *tabs = reinterpret_cast<unsigned long long *>(smem + (size_t)stages * stage_bytes);
     uint64_t *full = reinterpret_cast<uint64_t *>(tabs + (size_t)stages * NW * CS);
     uint64_t *empty = full + stages;
@@ -98,73 +185,43 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
     __syncthreads();
 
     if (warp == NW) {
-        // ===== producer warp: lane r < CS copies row r of the slab, lane CS copies the table slice =====
-        if (lane <= CS) {
-            const float *beam_in = in + (size_t)b * nchans * (size_t)nsamps;
-            const int32_t *rs = row_start + (size_t)blk * nslab * CS;
-            int st = 0;
-            uint32_t ph = 1;            // parity of the empty-barrier phase to wait for (first lap: no wait)
-            for (int slab = 0; slab < nslab; ++slab, ++st) {
-                if (st == stages) { st = 0; ph ^= 1; }
-                if (slab >= stages) mbar_wait(&empty[st], ph);
-                if (lane < CS) {
-                    const int c = slab * CS + lane;
-                    uint32_t bytes = 0;
-                    long long lo = 0, g0 = 0;
-                    if (c < nchans) {
-                        g0 = tile_t0 + rs[c];
-                        lo = g0 < 0 ? 0 : g0;
-                        long long hi = g0 + row_words;
-                        if (hi > nsamps) hi = nsamps;
-                        if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(float));
-                    }
-                    mbar_arrive_expect_tx(&full[st], bytes);
-                    if (bytes)
-                        bulk_g2s(rows + ((size_t)st * CS + lane) * row_words + (lo - g0), beam_in + (size_t)c * nsamps + lo, bytes,
-                                 &full[st]);
-                } else {
-                    const uint32_t bytes = NW * CS * sizeof(unsigned long long);
-                    mbar_arrive_expect_tx(&full[st], bytes);
-                    bulk_g2s(tabs + (size_t)st * NW * CS, warp_tab + ((size_t)blk * nslab + slab) * NW * CS, bytes, &full[st]);
-                }
-            }
-        }
+        if (lane <= CS)
+            producer_loop<float, NW, CS>(in + (size_t)b * nchans * (size_t)nsamps, row_start + (size_t)blk * nslab * CS,
+                                         warp_tab + (size_t)blk * nslab * NW * CS, smem, tabs, full, empty, tile_t0, nchans,
+                                         nslab, nsamps, row_words, stages, lane);
         return;
     }
 
     // ===== consumer warps =====
-    float acc[D][T];
+    unsigned long long acc[D][T / 2];
 #pragma unroll
     for (int j = 0; j < D; ++j)
 #pragma unroll
-        for (int i = 0; i < T; ++i) acc[j][i] = 0.f;
+        for (int i = 0; i < T / 2; ++i) acc[j][i] = 0ull;      // (+0.f, +0.f)
 
+    const uint32_t lane_base = smem_u32(smem) + lane * (T * 4);
     int st = 0;
     uint32_t ph = 0;
+#pragma unroll 1
     for (int slab = 0; slab < nslab; ++slab, ++st) {
         if (st == stages) { st = 0; ph ^= 1; }
         mbar_wait(&full[st], ph);
         const unsigned long long *tab = tabs + ((size_t)st * NW + warp) * CS;
-        const float4 *srow = reinterpret_cast<const float4 *>(rows + (size_t)st * CS * row_words) + lane * (T / 4);
+        const uint32_t sbase = lane_base + (uint32_t)(st * stage_bytes);
         const int nc = min(CS, nchans - slab * CS);
+        unsigned long long wt = tab[0];
+#pragma unroll 1
         for (int r = 0; r < nc; ++r) {
-            const unsigned long long wt = tab[r];
             const unsigned lo32 = (unsigned)wt, hi32 = (unsigned)(wt >> 32);
-            const float4 *p = srow + (size_t)r * (row_words / 4) + (lo32 & 0xffffu);
+            wt = tab[r + 1];                                  // prefetch (the entry after the last one is never used)
+            const uint32_t p = sbase + ((lo32 & 0xffffu) << 4);
             const int extra = (lo32 >> 16) & 0xf;
-            float w[W];
+            unsigned long long w[W2];
 #pragma unroll
-            for (int i = 0; i < W / 4; ++i) {
-                if (i < T / 4 || i - T / 4 < extra) {
-                    const float4 v = p[i];
-                    w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
-                }
-            }
+            for (int i = 0; i < T / 4; ++i) lds128(w[2 * i], w[2 * i + 1], p + 16 * i);
 #pragma unroll
-            for (int j = 0; j < D; ++j) {
-                const unsigned off = j == 0 ? (lo32 >> 24) : ((hi32 >> (8 * (j - 1))) & 0xffu);
-                VAdd<T, NOFF>::run(acc[j], w, off);
-            }
+            for (int i = T / 4; i < W2 / 2; ++i) lds128_if(w[2 * i], w[2 * i + 1], p + 16 * i, i - T / 4 < extra);
+            Chain::run(acc, w, lo32, hi32);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
@@ -176,19 +233,14 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
         const int dl = warp * D + j;
         const int d = blk * DB + dl;
         if (d >= ndms) continue;
-        const long long ts = tile_t0 - sigma[dl] + (long long)lane * T;
-        float *orow = out + ((size_t)b * ndms + d) * (size_t)nsamps;
+        float v[T];
 #pragma unroll
-        for (int i = 0; i < T; i += 4) {
-            const long long t = ts + i;
-            if (t >= 0 && t + 3 < nsamps_out) {
-                *reinterpret_cast<float4 *>(orow + t) = make_float4(acc[j][i], acc[j][i + 1], acc[j][i + 2], acc[j][i + 3]);
-            } else {
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (t + k >= 0 && t + k < nsamps_out) orow[t + k] = acc[j][i + k];
-            }
+        for (int i = 0; i < T / 2; ++i) {
+            v[2 * i] = __uint_as_float((unsigned)acc[j][i]);
+            v[2 * i + 1] = __uint_as_float((unsigned)(acc[j][i] >> 32));
         }
+        const long long ts = tile_t0 - sigma[dl] + (long long)lane * T;
+        store_row<T>(out + ((size_t)b * ndms + d) * (size_t)nsamps, ts, nsamps_out, v);
     }
 }
 
@@ -196,7 +248,9 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
 struct Geometry {
     int D, T, NW, CS, NOFF;
 };
-constexpr Geometry kGeomF32 = {4, 28, 11, 8, 16};
+// compiled fp32 geometries; index = plan option "tiled_geom"
+constexpr Geometry kGeomF32[] = {{4, 28, 11, 8, 12}, {4, 20, 15, 8, 12}, {5, 20, 11, 8, 16}, {4, 28, 11, 8, 16}};
+constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
 
 static inline long long floor4(long long v) { return v >= 0 ? (v / 4) * 4 : -(((-v) + 3) / 4) * 4; }
 
@@ -212,10 +266,9 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
     // un-rounded delay increment per DM step at the band edge: the slope the shear splits in half
     const double f_lo = p->f_top + (p->nchans - 1) * p->foff;
     const double smax = 4.148808e3 * p->dm_step * (1.0 / (f_lo * f_lo) - 1.0 / (p->f_top * p->f_top)) / p->tsamp;
-    bool found = false;
     int best_off = 1 << 30;
     double best_shear = 0.0;
-    const double cands[] = {0.5, 0.45, 0.55, 0.4, 0.6, 0.0};
+    const double cands[] = {0.5, 0.48, 0.52, 0.45, 0.55, 0.4, 0.6, 0.0};
     auto e_of = [&](int blk, int dl, int c, const std::vector<int32_t> &sig) -> long long {
         int d = blk * DB + dl;
         if (d >= p->ndms) d = p->ndms - 1;
@@ -223,7 +276,7 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
     };
     auto make_sigma = [&](double shear, std::vector<int32_t> &sig) {
         sig.resize(DB);
-        for (int dl = 0; dl < DB; ++dl) sig[dl] = (int32_t)(4 * llround(shear * smax * dl / 4.0));
+        for (int dl = 0; dl < DB; ++dl) sig[dl] = (int32_t)llround(shear * smax * dl);
     };
     for (double cand : cands) {
         std::vector<int32_t> sig;
@@ -242,11 +295,11 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
                 }
         if (worst < best_off) { best_off = worst; best_shear = cand; }
     }
-    found = best_off < g.NOFF;
-    if (!found) return false;
+    if (best_off >= g.NOFF) return false;
     make_sigma(best_shear, h_sigma);
     h_rs.assign((size_t)nblk * ncp, 0);
     h_tab.assign((size_t)nblk * nslab * g.NW * g.CS, 0ULL);
+    // pass 1: row starts and the longest staged row
     long long max_need = 0;
     for (int blk = 0; blk < nblk; ++blk)
         for (int c = 0; c < p->nchans; ++c) {
@@ -254,6 +307,24 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
             for (int dl = 0; dl < DB; ++dl) mn = std::min(mn, e_of(blk, dl, c, h_sigma));
             const long long rs = floor4(mn);
             h_rs[(size_t)blk * ncp + c] = (int32_t)rs;
+            for (int w = 0; w < g.NW; ++w) {
+                long long wmn = 1LL << 60, wmx = -(1LL << 60);
+                for (int j = 0; j < g.D; ++j) {
+                    const long long e = e_of(blk, w * g.D + j, c, h_sigma) - rs;
+                    wmn = std::min(wmn, e);
+                    wmx = std::max(wmx, e);
+                }
+                const long long A = floor4(wmn);
+                const int chunks = (g.T + (int)(wmx - A) + 3) / 4;
+                max_need = std::max(max_need, A + 31LL * g.T + 4LL * chunks);   // last word any lane of this warp touches
+            }
+        }
+    const int row_words = (int)((max_need + 3) / 4 * 4);
+    if ((long long)g.CS * row_words / 4 > 0xffff) return false;
+    // pass 2: the per-warp entries (window start includes the row's position in the stage)
+    for (int blk = 0; blk < nblk; ++blk)
+        for (int c = 0; c < p->nchans; ++c) {
+            const long long rs = h_rs[(size_t)blk * ncp + c];
             const int slab = c / g.CS, r = c % g.CS;
             for (int w = 0; w < g.NW; ++w) {
                 long long wmn = 1LL << 60, wmx = -(1LL << 60);
@@ -264,20 +335,16 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
                     wmx = std::max(wmx, e[j]);
                 }
                 const long long A = floor4(wmn);
-                const int maxoff = (int)(wmx - A);
-                const int chunks = (g.T + maxoff + 3) / 4;          // float4 chunks holding w[0 .. T+maxoff)
+                const int chunks = (g.T + (int)(wmx - A) + 3) / 4;       // 16-byte chunks holding w[0 .. T+maxoff)
                 const int extra = chunks - g.T / 4;
-                unsigned long long ent = (unsigned long long)(A / 4) | ((unsigned long long)extra << 16);
+                unsigned long long ent = (unsigned long long)((long long)r * row_words / 4 + A / 4) | ((unsigned long long)extra << 16);
                 for (int j = 0; j < g.D; ++j) ent |= (unsigned long long)(e[j] - A) << (24 + 8 * j);
                 h_tab[(((size_t)blk * nslab + slab) * g.NW + w) * g.CS + r] = ent;
-                // last word any lane of this warp touches in the row
-                max_need = std::max(max_need, A + 31LL * g.T + 4LL * chunks);
-                if (A / 4 > 0xffff) return false;
             }
         }
     tt.dms_per_warp = g.D; tt.warps = g.NW; tt.tpt = g.T;
     tt.dm_block = DB; tt.n_dm_blocks = nblk; tt.tile_t = TT;
-    tt.row_words = (int)((max_need + 3) / 4 * 4);
+    tt.row_words = row_words;
     tt.max_off = best_off;
     tt.sigma_max = *std::max_element(h_sigma.begin(), h_sigma.end());
     return true;
@@ -289,42 +356,19 @@ template <typename V> static bool upload(V **dptr, const std::vector<V> &h)
     return cudaMemcpy(*dptr, h.data(), h.size() * sizeof(V), cudaMemcpyHostToDevice) == cudaSuccess;
 }
 
-}  // namespace
-
-int mdsm_tiled_build_tables(mdsm_plan *p)
+static void free_tables(TiledTables *tt)
 {
-    p->tiled_f32.ok = false;
-    p->tiled_u8.ok = false;
-    if (p->nsamps % 4 != 0) return MDSM_OK;   // rows must be 16-byte aligned for the bulk copies
-    std::vector<int32_t> rs, sig;
-    std::vector<unsigned long long> tab;
-    TiledTables &tt = p->tiled_f32;
-    if (!build_tables(p, kGeomF32, tt, rs, tab, sig)) return MDSM_OK;
-    if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig)) {
-        mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
-        return MDSM_ECUDA;
-    }
-    tt.ok = true;
-    return MDSM_OK;
+    cudaFree(tt->d_row_start);
+    cudaFree(tt->d_warp_tab);
+    cudaFree(tt->d_sigma);
+    tt->d_row_start = nullptr; tt->d_warp_tab = nullptr; tt->d_sigma = nullptr;
+    tt->ok = false;
 }
 
-void mdsm_tiled_free_tables(mdsm_plan *p)
+template <int G>
+static int launch_f32(mdsm_plan *p, const TiledTables &tt, const float *d_in, int beam0, int nb, float *d_out, cudaStream_t st)
 {
-    for (TiledTables *tt : {&p->tiled_f32, &p->tiled_u8}) {
-        cudaFree(tt->d_row_start);
-        cudaFree(tt->d_warp_tab);
-        cudaFree(tt->d_sigma);
-        tt->d_row_start = nullptr; tt->d_warp_tab = nullptr; tt->d_sigma = nullptr;
-        tt->ok = false;
-    }
-}
-
-int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
-                                 cudaStream_t st)
-{
-    MDSM_REQUIRE(dtype == MDSM_F32, "tiled kernel: only MDSM_F32 so far");
-    const TiledTables &tt = p->tiled_f32;
-    constexpr Geometry g = kGeomF32;
+    constexpr Geometry g = kGeomF32[G];
     auto kern = dedisperse_tiled_f32_kernel<g.D, g.T, g.NW, g.CS, g.NOFF>;
     const int nslab = (p->nchans + g.CS - 1) / g.CS;
     const size_t stage_bytes = (size_t)g.CS * tt.row_words * sizeof(float) + (size_t)g.NW * g.CS * sizeof(unsigned long long);
@@ -332,7 +376,7 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
     if (stages > 8) stages = 8;
     if (stages > nslab) stages = nslab;
     MDSM_REQUIRE(stages >= 2 || nslab == 1, "tiled kernel: staged rows too large for shared memory");
-    const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t);
+    const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t) + 16;
     static thread_local size_t smem_set = 0;
     if (smem > smem_set) {
         MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -341,10 +385,55 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
     const long long ntile = (p->nsamps_out + tt.sigma_max + tt.tile_t - 1) / tt.tile_t;
     MDSM_REQUIRE(ntile <= 65535 && nb <= 65535, "tiled kernel: grid too large");
     dim3 grid(tt.n_dm_blocks, (unsigned)ntile, nb);
-    kern<<<grid, (g.NW + 1) * 32, smem, st>>>((const float *)d_in, (float *)d_out, tt.d_row_start,
-                                              (const unsigned long long *)tt.d_warp_tab, tt.d_sigma, beam0, p->nchans, nslab,
-                                              p->ndms, p->nsamps, p->nsamps_out, tt.row_words, stages);
+    kern<<<grid, (g.NW + 1) * 32, smem, st>>>(d_in, d_out, tt.d_row_start, (const unsigned long long *)tt.d_warp_tab, tt.d_sigma,
+                                              beam0, p->nchans, nslab, p->ndms, p->nsamps, p->nsamps_out, tt.row_words, stages);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 1;
     return MDSM_OK;
+}
+
+}  // namespace
+
+int mdsm_tiled_num_geoms(int dtype) { return dtype == MDSM_F32 ? kNumGeomF32 : 0; }
+
+int mdsm_tiled_build_tables(mdsm_plan *p)
+{
+    free_tables(&p->tiled_f32);
+    free_tables(&p->tiled_u8);
+    if (p->nsamps % 4 != 0) return MDSM_OK;   // rows must be 16-byte aligned for the bulk copies
+    std::vector<int32_t> rs, sig;
+    std::vector<unsigned long long> tab;
+    TiledTables &tt = p->tiled_f32;
+    if (p->tiled_geom_f32 < 0 || p->tiled_geom_f32 >= kNumGeomF32) return MDSM_OK;
+    if (!build_tables(p, kGeomF32[p->tiled_geom_f32], tt, rs, tab, sig)) return MDSM_OK;
+    if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig)) {
+        mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return MDSM_ECUDA;
+    }
+    tt.geom = p->tiled_geom_f32;
+    tt.ok = true;
+    return MDSM_OK;
+}
+
+void mdsm_tiled_free_tables(mdsm_plan *p)
+{
+    free_tables(&p->tiled_f32);
+    free_tables(&p->tiled_u8);
+}
+
+int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
+                                 cudaStream_t st)
+{
+    MDSM_REQUIRE(dtype == MDSM_F32, "tiled kernel: only MDSM_F32 so far");
+    const TiledTables &tt = p->tiled_f32;
+    const float *in = (const float *)d_in;
+    float *out = (float *)d_out;
+    switch (tt.geom) {
+        case 0: return launch_f32<0>(p, tt, in, beam0, nb, out, st);
+        case 1: return launch_f32<1>(p, tt, in, beam0, nb, out, st);
+        case 2: return launch_f32<2>(p, tt, in, beam0, nb, out, st);
+        case 3: return launch_f32<3>(p, tt, in, beam0, nb, out, st);
+    }
+    mdsm_set_error("tiled kernel: bad geometry index %d", tt.geom);
+    return MDSM_EINVAL;
 }

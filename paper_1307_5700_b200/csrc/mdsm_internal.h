@@ -38,6 +38,7 @@ struct TiledTables {
     void *d_warp_tab = nullptr;                   // [n_dm_blocks][nslab][warps][CS] packed window base + per-DM offsets
     int32_t *d_sigma = nullptr;                   // [n_dm_blocks*dm_block]  output time shear per DM
     int sigma_max = 0;
+    int geom = 0;                                 // index of the compiled geometry the tables were built for
     bool ok = false;
 };
 
@@ -60,6 +61,7 @@ struct mdsm_plan {
     double *d_series_stats = nullptr; // [nbeams][ndms][2] = mean, rms
 
     int dedisp_kernel = 0;            // 0 auto, 1 direct, 2 tiled
+    int tiled_geom_f32 = 0, tiled_geom_u8 = 0;   // compiled tile geometry per dtype (option "tiled_geom")
     TiledTables tiled_f32, tiled_u8;
 
     // host pipeline workspace (allocated on first mdsm_pipeline_host)
@@ -81,6 +83,7 @@ int mdsm_launch_dedisperse_direct(mdsm_plan *p, const void *d_in, int dtype, int
 int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
                                  cudaStream_t st);
 int mdsm_tiled_build_tables(mdsm_plan *p);
+int mdsm_tiled_num_geoms(int dtype);
 void mdsm_tiled_free_tables(mdsm_plan *p);
 int mdsm_launch_detect(mdsm_plan *p, const void *d_out, int dtype, int beam0, int nb, double snr_thresh,
                        mdsm_event *d_events, int64_t max_events, unsigned long long *d_count, cudaStream_t st);

@@ -56,6 +56,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "}" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
+// producer-side wait: the producer runs several stages ahead, so it sleeps between polls instead of
+// spinning (a spinning producer warp took 12 % of the SM's issue slots in the r1b profile)
+__device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    for (;;) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(256);
+    }
+}
 __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
@@ -124,7 +140,7 @@ __device__ __forceinline__ void producer_loop(const TIn *__restrict__ beam_in, c
     uint32_t ph = 1;            // parity of the empty-barrier phase to wait for (first lap: no wait)
     for (int slab = 0; slab < nslab; ++slab, ++st) {
         if (st == stages) { st = 0; ph ^= 1; }
-        if (slab >= stages) mbar_wait(&empty[st], ph);
+        if (slab >= stages) mbar_wait_sleep(&empty[st], ph);
         if (lane < CS) {
             const int c = slab * CS + lane;
             uint32_t bytes = 0;

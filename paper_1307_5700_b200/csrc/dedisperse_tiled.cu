@@ -3,24 +3,31 @@
 //   out[b][d][t] = sum_c in[b][c][t + delay(d,c)]
 //
 // Work decomposition:
-//   CTA   = one beam x one block of DB = NW*D consecutive DM trials x one time tile of 32*T samples.
+//   tile  = one beam x one block of DB = NW*D consecutive DM trials x one time tile of 32*T samples.
+//   CTA   = persistent: one per SM, walks tiles (DM block fastest, so that the CTAs running together
+//           read the same input rows out of L2) and, inside a tile, the channel PARTS (u8 only: <= 256
+//           channels, the most a 16-bit lane can hold) and the channel SLABS of a part.
 //   warp  = D consecutive DM trials of the block, all 32*T samples of the tile.
 //   thread= D x T accumulators in registers: T CONSECUTIVE samples (lane*T ...) of each of its D DMs.
 // Per channel a thread loads ONE register window of T + (spread of its D delays) consecutive samples
-// from shared memory with conflict-free 128-bit loads (T/4 is odd) and adds it, at D different
-// register offsets, into its D accumulator rows -- every shared-memory word feeds ~3 adds, which is
-// what lifts the kernel off the 32 words/clk/SM shared-memory ceiling (25 % of the add peak).
-// The offsets are warp-uniform; they select straight-line add blocks through a threaded chain of
-// indirect branches (chain_gen.h).  fp32 accumulators and window are packed f32x2 register pairs so
-// that an even offset costs T/2 issue slots (FADD2) -- the FMA pipe, not the issue port, is the limit.
+// from shared memory with conflict-free 128-bit loads and adds it, at D different register offsets, into
+// its D accumulator rows -- every shared-memory word feeds ~3 adds, which is what lifts the kernel off the
+// 32 words/clk/SM shared-memory ceiling (25 % of the add peak).  The offsets are warp-uniform; they select
+// straight-line add blocks through a threaded chain of indirect branches (chain_gen.h, gen_chain.py).
+//   fp32: accumulators and window are packed f32x2 register pairs (FADD2 for even offsets).
+//   u8  : the input is widened once to u16 (plan scratch); accumulators are packed u16x2 lanes (one add =
+//         two samples), flushed into the uint32 output after every part (part 0 stores, later parts
+//         read-modify-write their own elements, which are still in L2).
 // The time axis is SHEARED: DM d of a block owns outputs [tile_t0 - sigma_d, tile_t0 - sigma_d + 32T)
-// with sigma_d ~ half the band-edge delay slope, which halves the spread of the D windows (and of
-// the staged rows) compared with an unsheared tile.
-// Staging: a producer warp streams channel slabs (CS rows of `row_words` samples, each starting at
-// its own 16-byte-aligned delay-dependent offset) into a ring of shared-memory stages with 1-D TMA
-// bulk copies (cp.async.bulk ... mbarrier::complete_tx), full/empty mbarriers per stage.
+// with sigma_d ~ half the band-edge delay slope, which halves the spread of the D windows (and of the
+// staged rows) compared with an unsheared tile.
+// Staging: a producer warp streams channel slabs (CS rows of `row_elems` samples, each starting at its own
+// 16-byte-aligned delay-dependent offset) into a ring of shared-memory stages with 1-D TMA bulk copies
+// (cp.async.bulk ... mbarrier::complete_tx), full/empty mbarriers per stage; it runs ahead across tile
+// boundaries, so a CTA never drains its pipeline between tiles.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <vector>
 
 #include "chain_gen.h"
@@ -44,33 +51,26 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t by
     asm volatile("{ .reg .b64 t; mbarrier.arrive.expect_tx.shared::cta.b64 t, [%0], %1; }" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
 {
+    uint32_t done;
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
-        "W: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra D;\n\t"
-        "bra W;\n\t"
-        "D:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return done != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
 }
 // producer-side wait: the producer runs several stages ahead, so it sleeps between polls instead of
 // spinning (a spinning producer warp took 12 % of the SM's issue slots in the r1b profile)
 __device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity)
 {
-    uint32_t done;
-    for (;;) {
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t"
-            "}" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(256);
-    }
+    while (!mbar_try_wait(bar, parity)) __nanosleep(256);
 }
 __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
 {
@@ -78,26 +78,17 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void lds128(unsigned long long &a, unsigned long long &b, uint32_t addr)
-{
-    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
-}
 
-// predicated form: one SASS instruction, no branch (the registers keep stale data when pred is false)
-__device__ __forceinline__ void lds128_if(unsigned long long &a, unsigned long long &b, uint32_t addr, bool pred)
-{
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q ld.shared.v2.b64 {%0, %1}, [%2]; }" : "=l"(a), "=l"(b) : "r"(addr), "r"((unsigned)pred));
-}
-
-// Stores v[0..T) to orow[ts .. ts+T), clipped to [0, n).  Rows are 16-byte aligned; ts is not (the
-// shear is a whole number of samples), so the head up to the next multiple of 4 goes out as scalars and
-// the rest as 128-bit stores.  The head length is warp-uniform: one switch, static register indexing.
-template <int T, int H, typename V>
+// Writes v[0..T) to orow[ts .. ts+T), clipped to [0, n); ACCUM adds to what is there (the elements are
+// this thread's own: no other thread of the launch touches them).  Rows are 16-byte aligned; ts is not (the
+// shear is a whole number of samples), so the head up to the next multiple of 4 goes out as scalars and the
+// rest as 128-bit accesses.  The head length is warp-uniform: one switch, static register indexing.
+template <int T, int H, bool ACCUM, typename V>
 __device__ __forceinline__ void store_row_h(V *orow, long long ts, long long n, const V (&v)[T])
 {
 #pragma unroll
     for (int i = 0; i < H; ++i)
-        if (ts + i >= 0 && ts + i < n) orow[ts + i] = v[i];
+        if (ts + i >= 0 && ts + i < n) orow[ts + i] = ACCUM ? (V)(orow[ts + i] + v[i]) : v[i];
 #pragma unroll
     for (int i = H; i + 3 < T; i += 4) {
         const long long t = ts + i;
@@ -105,92 +96,94 @@ __device__ __forceinline__ void store_row_h(V *orow, long long ts, long long n, 
             uint4 q;
             q.x = reinterpret_cast<const uint32_t &>(v[i]); q.y = reinterpret_cast<const uint32_t &>(v[i + 1]);
             q.z = reinterpret_cast<const uint32_t &>(v[i + 2]); q.w = reinterpret_cast<const uint32_t &>(v[i + 3]);
+            if (ACCUM) {                                   // integer path only (uint32 adds)
+                const uint4 o = *reinterpret_cast<const uint4 *>(orow + t);
+                q.x += o.x; q.y += o.y; q.z += o.z; q.w += o.w;
+            }
             *reinterpret_cast<uint4 *>(orow + t) = q;
         } else {
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-                if (t + k >= 0 && t + k < n) orow[t + k] = v[i + k];
+                if (t + k >= 0 && t + k < n) orow[t + k] = ACCUM ? (V)(orow[t + k] + v[i + k]) : v[i + k];
         }
     }
 #pragma unroll
     for (int i = H + (T - H) / 4 * 4; i < T; ++i)
-        if (ts + i >= 0 && ts + i < n) orow[ts + i] = v[i];
+        if (ts + i >= 0 && ts + i < n) orow[ts + i] = ACCUM ? (V)(orow[ts + i] + v[i]) : v[i];
 }
-template <int T, typename V>
+template <int T, bool ACCUM, typename V>
 __device__ __forceinline__ void store_row(V *orow, long long ts, long long n, const V (&v)[T])
 {
     static_assert(sizeof(V) == 4, "32-bit outputs");
     switch ((int)((4 - (ts & 3)) & 3)) {
-        case 0: store_row_h<T, 0>(orow, ts, n, v); break;
-        case 1: store_row_h<T, 1>(orow, ts, n, v); break;
-        case 2: store_row_h<T, 2>(orow, ts, n, v); break;
-        default: store_row_h<T, 3>(orow, ts, n, v); break;
+        case 0: store_row_h<T, 0, ACCUM>(orow, ts, n, v); break;
+        case 1: store_row_h<T, 1, ACCUM>(orow, ts, n, v); break;
+        case 2: store_row_h<T, 2, ACCUM>(orow, ts, n, v); break;
+        default: store_row_h<T, 3, ACCUM>(orow, ts, n, v); break;
     }
 }
 
-// ------------------------------------------------------------------ producer (shared by the dtypes)
-// Lane r < CS copies row r of every slab, lane CS copies the slab's slice of the warp table.
-template <typename TIn, int NW, int CS>
-__device__ __forceinline__ void producer_loop(const TIn *__restrict__ beam_in, const int32_t *__restrict__ rs,
-                                              const unsigned long long *__restrict__ wtab, unsigned char *rows,
-                                              unsigned long long *tabs, uint64_t *full, uint64_t *empty, long long tile_t0,
-                                              int nchans, int nslab, long long nsamps, int row_elems, int stages, int lane)
-{
-    int st = 0;
-    uint32_t ph = 1;            // parity of the empty-barrier phase to wait for (first lap: no wait)
-    for (int slab = 0; slab < nslab; ++slab, ++st) {
-        if (st == stages) { st = 0; ph ^= 1; }
-        if (slab >= stages) mbar_wait_sleep(&empty[st], ph);
-        if (lane < CS) {
-            const int c = slab * CS + lane;
-            uint32_t bytes = 0;
-            long long lo = 0, g0 = 0;
-            if (c < nchans) {
-                g0 = tile_t0 + rs[c];
-                lo = g0 < 0 ? 0 : g0;
-                long long hi = g0 + row_elems;
-                if (hi > nsamps) hi = nsamps;
-                if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(TIn));
-            }
-            mbar_arrive_expect_tx(&full[st], bytes);
-            if (bytes)
-                bulk_g2s(rows + (((size_t)st * CS + lane) * row_elems + (lo - g0)) * sizeof(TIn),
-                         beam_in + (size_t)c * nsamps + lo, bytes, &full[st]);
-        } else if (lane == CS) {
-            const uint32_t bytes = NW * CS * sizeof(unsigned long long);
-            mbar_arrive_expect_tx(&full[st], bytes);
-            bulk_g2s(tabs + (size_t)st * NW * CS, wtab + (size_t)slab * NW * CS, bytes, &full[st]);
-        }
+// tile index -> (DM block, time tile, beam); DM block fastest
+struct TileWalk {
+    int nblk, ntile_t;
+    long long ntiles;
+    __device__ __forceinline__ void decode(long long tile, int &blk, int &tt, int &bb) const
+    {
+        blk = (int)(tile % nblk);
+        const long long rest = tile / nblk;
+        tt = (int)(rest % ntile_t);
+        bb = (int)(rest / ntile_t);
     }
-}
+};
 
-// ------------------------------------------------------------------ fp32 kernel
-// warp_tab entry (64 bit): bits 0..15 window start in 16-byte units relative to the stage base (row r
-// included), bits 16..19 number of 16-byte chunks to load beyond T/4 (adaptive window), byte 3+j:
-// register offset of DM j.
-template <int D, int T, int NW, int CS, int NOFF>
-__global__ void __launch_bounds__((NW + 1) * 32, 1)
-dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ out, const int32_t *__restrict__ row_start,
-                            const unsigned long long *__restrict__ warp_tab, const int32_t *__restrict__ sigma, int beam0,
-                            int nchans, int nslab, int ndms, long long nsamps, long long nsamps_out, int row_words,
-                            int stages)
+struct TiledArgs {
+    const void *in;
+    void *out;
+    const int32_t *row_start;             // [nblk][nslab*CS]  first staged sample of the row, relative to tile_t0
+    const unsigned long long *warp_tab;   // [nblk][nslab][NW][CS] window entries (format: gen_chain.py)
+    const int32_t *sigma;                 // [DB] output time shear per DM of a block
+    int beam0, nchans, nslab, slabs_per_part, ndms;
+    long long nsamps, nsamps_out;
+    int row_elems, stages;
+    TileWalk walk;
+};
+
+template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
+    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, NOFF = NOFF_, AW = T_ / 2;
+    static constexpr bool kF32 = true;
+    using In = float; using Out = float; using Acc = unsigned long long;
+    using Slab = SlabF32<D_, T_, NOFF_>;
+    static_assert(T_ % 4 == 0 && (T_ / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
+};
+template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
+    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, NOFF = NOFF_, AW = T_ / 2;
+    static constexpr bool kF32 = false;
+    using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
+    using Slab = SlabU16<D_, T_, NOFF_>;
+    static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
+};
+
+// ------------------------------------------------------------------ the kernel
+template <typename Tr>
+__global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(const TiledArgs a)
 {
-    static_assert(T % 4 == 0 && (T / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
-    static_assert(D <= 5, "table entry holds at most 5 offsets");
-    using Chain = ChainF32<D, T, NOFF>;
-    constexpr int W2 = Chain::W2;           // window length in f32x2 pairs
-    constexpr int DB = D * NW;
+    using In = typename Tr::In;
+    using Out = typename Tr::Out;
+    using Acc = typename Tr::Acc;
+    constexpr int D = Tr::D, T = Tr::T, NW = Tr::NW, CS = Tr::CS, AW = Tr::AW, DB = D * NW;
     extern __shared__ __align__(128) unsigned char smem[];
-    const size_t stage_bytes = (size_t)CS * row_words * sizeof(float);
+    const int stages = a.stages;
+    const uint32_t stage_bytes = (uint32_t)CS * a.row_elems * sizeof(In);
     unsigned long long *tabs = reinterpret_cast<unsigned long long *>(smem + (size_t)stages * stage_bytes);
     uint64_t *full = reinterpret_cast<uint64_t *>(tabs + (size_t)stages * NW * CS);
     uint64_t *empty = full + stages;
-
-    const int blk = blockIdx.x;
-    const long long tile_t0 = (long long)blockIdx.y * (32 * T);
-    const int b = beam0 + blockIdx.z;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
+    // Rows that stick out of [0, nsamps) are only partly written by the bulk copies.  What they leave behind
+    // feeds outputs outside [0, nsamps_out) only, but a stale 16-bit lane must never carry into its valid
+    // neighbour: with the stages zeroed once, every staged value is zero or a real sample.
+    for (uint32_t i = threadIdx.x; i < stages * stage_bytes / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], CS + 1);
@@ -200,63 +193,112 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
     }
     __syncthreads();
 
+    const int ncp = a.nslab * CS;
     if (warp == NW) {
-        if (lane <= CS)
-            producer_loop<float, NW, CS>(in + (size_t)b * nchans * (size_t)nsamps, row_start + (size_t)blk * nslab * CS,
-                                         warp_tab + (size_t)blk * nslab * NW * CS, smem, tabs, full, empty, tile_t0, nchans,
-                                         nslab, nsamps, row_words, stages, lane);
+        // ===== producer: lane r < CS copies row r of every slab, lane CS the slab's slice of the warp table =====
+        if (lane > CS) return;
+        int st = 0;
+        uint32_t ph = 1;             // parity of the empty-barrier phase to wait for (first lap: no wait)
+        bool first_lap = true;
+        for (long long tile = blockIdx.x; tile < a.walk.ntiles; tile += gridDim.x) {
+            int blk, tt, bb;
+            a.walk.decode(tile, blk, tt, bb);
+            const long long tile_t0 = (long long)tt * (32 * T);
+            const In *beam_in = reinterpret_cast<const In *>(a.in) + (size_t)(a.beam0 + bb) * a.nchans * (size_t)a.nsamps;
+            const int32_t *rs = a.row_start + (size_t)blk * ncp;
+            const unsigned long long *wt = a.warp_tab + (size_t)blk * a.nslab * NW * CS;
+            for (int slab = 0; slab < a.nslab; ++slab) {
+                if (!first_lap) mbar_wait_sleep(&empty[st], ph);
+                if (lane < CS) {
+                    const int c = slab * CS + lane;
+                    uint32_t bytes = 0;
+                    long long lo = 0, g0 = 0;
+                    if (c < a.nchans) {
+                        g0 = tile_t0 + rs[c];
+                        lo = g0 < 0 ? 0 : g0;
+                        long long hi = g0 + a.row_elems;
+                        if (hi > a.nsamps) hi = a.nsamps;
+                        if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(In));
+                    }
+                    mbar_arrive_expect_tx(&full[st], bytes);
+                    if (bytes)
+                        bulk_g2s(smem + (size_t)st * stage_bytes + ((size_t)lane * a.row_elems + (lo - g0)) * sizeof(In),
+                                 beam_in + (size_t)c * a.nsamps + lo, bytes, &full[st]);
+                } else {
+                    const uint32_t bytes = NW * CS * sizeof(unsigned long long);
+                    mbar_arrive_expect_tx(&full[st], bytes);
+                    bulk_g2s(tabs + (size_t)st * NW * CS, wt + (size_t)slab * NW * CS, bytes, &full[st]);
+                }
+                if (++st == stages) { st = 0; ph ^= 1; first_lap = false; }
+            }
+        }
         return;
     }
 
     // ===== consumer warps =====
-    unsigned long long acc[D][T / 2];
-#pragma unroll
-    for (int j = 0; j < D; ++j)
-#pragma unroll
-        for (int i = 0; i < T / 2; ++i) acc[j][i] = 0ull;      // (+0.f, +0.f)
-
-    const uint32_t lane_base = smem_u32(smem) + lane * (T * 4);
+    Acc acc[D][AW];
+    const uint32_t lane_base = smem_u32(smem) + lane * (T * (uint32_t)sizeof(In));
+    const uint32_t tab_base = smem_u32(tabs) + warp * (CS * 8);
     int st = 0;
     uint32_t ph = 0;
+    for (long long tile = blockIdx.x; tile < a.walk.ntiles; tile += gridDim.x) {
+        int blk, tt, bb;
+        a.walk.decode(tile, blk, tt, bb);
+        const long long tile_t0 = (long long)tt * (32 * T);
+        const int b = a.beam0 + bb;
 #pragma unroll 1
-    for (int slab = 0; slab < nslab; ++slab, ++st) {
-        if (st == stages) { st = 0; ph ^= 1; }
-        mbar_wait(&full[st], ph);
-        const unsigned long long *tab = tabs + ((size_t)st * NW + warp) * CS;
-        const uint32_t sbase = lane_base + (uint32_t)(st * stage_bytes);
-        const int nc = min(CS, nchans - slab * CS);
-        unsigned long long wt = tab[0];
+        for (int s0 = 0; s0 < a.nslab; s0 += a.slabs_per_part) {
+#pragma unroll
+            for (int j = 0; j < D; ++j)
+#pragma unroll
+                for (int i = 0; i < AW; ++i) acc[j][i] = 0;      // (+0.f, +0.f) / (0, 0)
+            const int s1 = min(a.nslab, s0 + a.slabs_per_part);
 #pragma unroll 1
-        for (int r = 0; r < nc; ++r) {
-            const unsigned lo32 = (unsigned)wt, hi32 = (unsigned)(wt >> 32);
-            wt = tab[r + 1];                                  // prefetch (the entry after the last one is never used)
-            const uint32_t p = sbase + ((lo32 & 0xffffu) << 4);
-            const int extra = (lo32 >> 16) & 0xf;
-            unsigned long long w[W2];
+            for (int slab = s0; slab < s1; ++slab) {
+                mbar_wait(&full[st], ph);
+                Tr::Slab::run(acc, lane_base + st * stage_bytes, tab_base + st * (NW * CS * 8));
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
+                if (++st == stages) { st = 0; ph ^= 1; }
+            }
+            // ----- epilogue of the part: each thread owns T consecutive outputs of each of its D DMs -----
 #pragma unroll
-            for (int i = 0; i < T / 4; ++i) lds128(w[2 * i], w[2 * i + 1], p + 16 * i);
+            for (int j = 0; j < D; ++j) {
+                const int dl = warp * D + j;
+                const int d = blk * DB + dl;
+                if (d >= a.ndms) continue;
+                Out v[T];
 #pragma unroll
-            for (int i = T / 4; i < W2 / 2; ++i) lds128_if(w[2 * i], w[2 * i + 1], p + 16 * i, i - T / 4 < extra);
-            Chain::run(acc, w, lo32, hi32);
+                for (int i = 0; i < AW; ++i) {
+                    if constexpr (Tr::kF32) {
+                        v[2 * i] = __uint_as_float((unsigned)acc[j][i]);
+                        v[2 * i + 1] = __uint_as_float((unsigned)(acc[j][i] >> 32));
+                    } else {
+                        v[2 * i] = acc[j][i] & 0xffffu;
+                        v[2 * i + 1] = acc[j][i] >> 16;
+                    }
+                }
+                const long long ts = tile_t0 - a.sigma[dl] + (long long)lane * T;
+                Out *orow = reinterpret_cast<Out *>(a.out) + ((size_t)b * a.ndms + d) * (size_t)a.nsamps;
+                if (Tr::kF32 || s0 == 0) store_row<T, false>(orow, ts, a.nsamps_out, v);
+                else store_row<T, true>(orow, ts, a.nsamps_out, v);
+            }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);
     }
+}
 
-    // ===== epilogue: each thread owns T consecutive outputs of each of its D DMs =====
-#pragma unroll
-    for (int j = 0; j < D; ++j) {
-        const int dl = warp * D + j;
-        const int d = blk * DB + dl;
-        if (d >= ndms) continue;
-        float v[T];
-#pragma unroll
-        for (int i = 0; i < T / 2; ++i) {
-            v[2 * i] = __uint_as_float((unsigned)acc[j][i]);
-            v[2 * i + 1] = __uint_as_float((unsigned)(acc[j][i] >> 32));
-        }
-        const long long ts = tile_t0 - sigma[dl] + (long long)lane * T;
-        store_row<T>(out + ((size_t)b * ndms + d) * (size_t)nsamps, ts, nsamps_out, v);
+// widens the uint8 filterbank to uint16 (the staged element type of the integer kernel)
+__global__ void __launch_bounds__(256) widen_u8_kernel(const uint4 *__restrict__ in, uint4 *__restrict__ out, size_t n16)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 v = in[i];
+        uint4 a, b;
+        a.x = __byte_perm(v.x, 0, 0x4140); a.y = __byte_perm(v.x, 0, 0x4342);
+        a.z = __byte_perm(v.y, 0, 0x4140); a.w = __byte_perm(v.y, 0, 0x4342);
+        b.x = __byte_perm(v.z, 0, 0x4140); b.y = __byte_perm(v.z, 0, 0x4342);
+        b.z = __byte_perm(v.w, 0, 0x4140); b.w = __byte_perm(v.w, 0, 0x4342);
+        out[2 * i] = a;
+        out[2 * i + 1] = b;
     }
 }
 
@@ -264,15 +306,19 @@ dedisperse_tiled_f32_kernel(const float *__restrict__ in, float *__restrict__ ou
 struct Geometry {
     int D, T, NW, CS, NOFF;
 };
-// compiled fp32 geometries; index = plan option "tiled_geom"
-constexpr Geometry kGeomF32[] = {{4, 28, 11, 8, 12}, {4, 20, 15, 8, 12}, {5, 20, 11, 8, 16}, {4, 28, 11, 8, 16}};
+// compiled geometries; index = plan option "tiled_geom_<dtype>"
+constexpr Geometry kGeomF32[] = {{4, 28, 11, 8, 12}, {4, 20, 15, 8, 12}};
+constexpr Geometry kGeomU16[] = {{4, 40, 11, 8, 16}};
 constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
+constexpr int kNumGeomU16 = sizeof(kGeomU16) / sizeof(kGeomU16[0]);
+constexpr int kPartChansU16 = 256;          // 256 * 255 < 2^16: the most channels a 16-bit lane can take
 
-static inline long long floor4(long long v) { return v >= 0 ? (v / 4) * 4 : -(((-v) + 3) / 4) * 4; }
+static inline long long floor_to(long long v, int a) { return v >= 0 ? (v / a) * a : -(((-v) + a - 1) / a) * a; }
 
-// Builds the row-start / per-warp window tables for one geometry.  Returns false if this plan's
-// delay spread does not fit the geometry's register window (the caller then uses the direct kernel).
-static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt, std::vector<int32_t> &h_rs,
+// Builds the row-start / per-warp window tables for one geometry.  `al` = samples per 16 bytes of the staged
+// element type.  Returns false if this plan's delay spread does not fit the geometry's register window (the
+// caller then uses the direct kernel).
+static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, TiledTables &tt, std::vector<int32_t> &h_rs,
                          std::vector<unsigned long long> &h_tab, std::vector<int32_t> &h_sigma)
 {
     const int DB = g.D * g.NW, TT = 32 * g.T;
@@ -307,7 +353,7 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
                         mn = std::min(mn, e);
                         mx = std::max(mx, e);
                     }
-                    worst = std::max(worst, (int)(mx - floor4(mn)));
+                    worst = std::max(worst, (int)(mx - floor_to(mn, al)));
                 }
         if (worst < best_off) { best_off = worst; best_shear = cand; }
     }
@@ -321,7 +367,7 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
         for (int c = 0; c < p->nchans; ++c) {
             long long mn = 1LL << 60;
             for (int dl = 0; dl < DB; ++dl) mn = std::min(mn, e_of(blk, dl, c, h_sigma));
-            const long long rs = floor4(mn);
+            const long long rs = floor_to(mn, al);
             h_rs[(size_t)blk * ncp + c] = (int32_t)rs;
             for (int w = 0; w < g.NW; ++w) {
                 long long wmn = 1LL << 60, wmx = -(1LL << 60);
@@ -330,18 +376,20 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
                     wmn = std::min(wmn, e);
                     wmx = std::max(wmx, e);
                 }
-                const long long A = floor4(wmn);
-                const int chunks = (g.T + (int)(wmx - A) + 3) / 4;
-                max_need = std::max(max_need, A + 31LL * g.T + 4LL * chunks);   // last word any lane of this warp touches
+                const long long A = floor_to(wmn, al);
+                const int chunks = (g.T + (int)(wmx - A) + al - 1) / al;
+                max_need = std::max(max_need, A + 31LL * g.T + (long long)al * chunks);   // last sample any lane of this warp touches
             }
         }
-    const int row_words = (int)((max_need + 3) / 4 * 4);
-    if ((long long)g.CS * row_words / 4 > 0xffff) return false;
+    const int row_elems = (int)((max_need + al - 1) / al * al);
+    const int esize = 16 / al;
+    if ((long long)g.CS * row_elems * esize >= (1 << 18)) return false;      // entry holds an 18-bit byte offset
     // pass 2: the per-warp entries (window start includes the row's position in the stage)
     for (int blk = 0; blk < nblk; ++blk)
         for (int c = 0; c < p->nchans; ++c) {
             const long long rs = h_rs[(size_t)blk * ncp + c];
             const int slab = c / g.CS, r = c % g.CS;
+            const bool last = (r == g.CS - 1) || (c == p->nchans - 1);
             for (int w = 0; w < g.NW; ++w) {
                 long long wmn = 1LL << 60, wmx = -(1LL << 60);
                 long long e[8];
@@ -350,17 +398,21 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, TiledTables &tt,
                     wmn = std::min(wmn, e[j]);
                     wmx = std::max(wmx, e[j]);
                 }
-                const long long A = floor4(wmn);
-                const int chunks = (g.T + (int)(wmx - A) + 3) / 4;       // 16-byte chunks holding w[0 .. T+maxoff)
-                const int extra = chunks - g.T / 4;
-                unsigned long long ent = (unsigned long long)((long long)r * row_words / 4 + A / 4) | ((unsigned long long)extra << 16);
-                for (int j = 0; j < g.D; ++j) ent |= (unsigned long long)(e[j] - A) << (24 + 8 * j);
-                h_tab[(((size_t)blk * nslab + slab) * g.NW + w) * g.CS + r] = ent;
+                const long long A = floor_to(wmn, al);
+                const int chunks = (g.T + (int)(wmx - A) + al - 1) / al;       // 16-byte chunks holding w[0 .. T+maxoff)
+                const int extra = chunks - g.T / al;
+                unsigned long long lo = (unsigned long long)(((long long)r * row_elems + A) * esize);
+                for (int i = 0; i < extra; ++i) lo |= 1ULL << (28 + i);
+                if (last) lo |= 1ULL << 31;
+                unsigned long long hi = 0;
+                static const char *dbg_force = getenv("MDSM_DEBUG_FORCE_OFFSET");   // experiments only: wrong results
+                for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(dbg_force ? atoi(dbg_force) : (e[j] - A)) << (8 * j);
+                h_tab[(((size_t)blk * nslab + slab) * g.NW + w) * g.CS + r] = lo | (hi << 32);
             }
         }
-    tt.dms_per_warp = g.D; tt.warps = g.NW; tt.tpt = g.T;
+    tt.dms_per_warp = g.D; tt.warps = g.NW; tt.tpt = g.T; tt.cs = g.CS;
     tt.dm_block = DB; tt.n_dm_blocks = nblk; tt.tile_t = TT;
-    tt.row_words = row_words;
+    tt.row_words = row_elems;
     tt.max_off = best_off;
     tt.sigma_max = *std::max_element(h_sigma.begin(), h_sigma.end());
     return true;
@@ -381,53 +433,79 @@ static void free_tables(TiledTables *tt)
     tt->ok = false;
 }
 
-template <int G>
-static int launch_f32(mdsm_plan *p, const TiledTables &tt, const float *d_in, int beam0, int nb, float *d_out, cudaStream_t st)
+template <typename Tr>
+static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, int beam0, int nb, void *d_out, int part_chans,
+                        cudaStream_t st)
 {
-    constexpr Geometry g = kGeomF32[G];
-    auto kern = dedisperse_tiled_f32_kernel<g.D, g.T, g.NW, g.CS, g.NOFF>;
-    const int nslab = (p->nchans + g.CS - 1) / g.CS;
-    const size_t stage_bytes = (size_t)g.CS * tt.row_words * sizeof(float) + (size_t)g.NW * g.CS * sizeof(unsigned long long);
+    auto kern = dedisperse_tiled_kernel<Tr>;
+    const int nslab = (p->nchans + Tr::CS - 1) / Tr::CS;
+    const size_t stage_bytes = (size_t)Tr::CS * tt.row_words * sizeof(typename Tr::In) + (size_t)Tr::NW * Tr::CS * sizeof(unsigned long long);
     int stages = (int)((220 * 1024 - 256) / stage_bytes);
-    if (stages > 8) stages = 8;
-    if (stages > nslab) stages = nslab;
-    MDSM_REQUIRE(stages >= 2 || nslab == 1, "tiled kernel: staged rows too large for shared memory");
+    if (stages > 12) stages = 12;
+    MDSM_REQUIRE(stages >= 2, "tiled kernel: staged rows too large for shared memory");
     const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t) + 16;
+    int cur = 0;
     static thread_local size_t smem_set = 0;
     if (smem > smem_set) {
         MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         smem_set = smem;
     }
-    const long long ntile = (p->nsamps_out + tt.sigma_max + tt.tile_t - 1) / tt.tile_t;
-    MDSM_REQUIRE(ntile <= 65535 && nb <= 65535, "tiled kernel: grid too large");
-    dim3 grid(tt.n_dm_blocks, (unsigned)ntile, nb);
-    kern<<<grid, (g.NW + 1) * 32, smem, st>>>(d_in, d_out, tt.d_row_start, (const unsigned long long *)tt.d_warp_tab, tt.d_sigma,
-                                              beam0, p->nchans, nslab, p->ndms, p->nsamps, p->nsamps_out, tt.row_words, stages);
+    (void)cur;
+    TiledArgs a;
+    a.in = d_in; a.out = d_out;
+    a.row_start = tt.d_row_start; a.warp_tab = (const unsigned long long *)tt.d_warp_tab; a.sigma = tt.d_sigma;
+    a.beam0 = beam0; a.nchans = p->nchans; a.nslab = nslab; a.ndms = p->ndms;
+    a.slabs_per_part = part_chans > 0 ? part_chans / Tr::CS : nslab;
+    a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out;
+    a.row_elems = tt.row_words; a.stages = stages;
+    a.walk.nblk = tt.n_dm_blocks;
+    a.walk.ntile_t = (int)((p->nsamps_out + tt.sigma_max + tt.tile_t - 1) / tt.tile_t);
+    a.walk.ntiles = (long long)a.walk.nblk * a.walk.ntile_t * nb;
+    const int grid = (int)std::min<long long>(a.walk.ntiles, p->sm_count);
+    kern<<<grid, (Tr::NW + 1) * 32, smem, st>>>(a);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 1;
     return MDSM_OK;
 }
 
+template <int G> using GeomF32 = TraitsF32<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
+template <int G> using GeomU16 = TraitsU16<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
+
+static int build_one(mdsm_plan *p, const Geometry &g, int al, int geom, TiledTables &tt)
+{
+    std::vector<int32_t> rs, sig;
+    std::vector<unsigned long long> tab;
+    if (!build_tables(p, g, al, tt, rs, tab, sig)) return MDSM_OK;
+    if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig)) {
+        mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return MDSM_ECUDA;
+    }
+    tt.geom = geom;
+    tt.ok = true;
+    return MDSM_OK;
+}
+
 }  // namespace
 
-int mdsm_tiled_num_geoms(int dtype) { return dtype == MDSM_F32 ? kNumGeomF32 : 0; }
+int mdsm_tiled_num_geoms(int dtype) { return dtype == MDSM_F32 ? kNumGeomF32 : kNumGeomU16; }
 
 int mdsm_tiled_build_tables(mdsm_plan *p)
 {
     free_tables(&p->tiled_f32);
     free_tables(&p->tiled_u8);
-    if (p->nsamps % 4 != 0) return MDSM_OK;   // rows must be 16-byte aligned for the bulk copies
-    std::vector<int32_t> rs, sig;
-    std::vector<unsigned long long> tab;
-    TiledTables &tt = p->tiled_f32;
-    if (p->tiled_geom_f32 < 0 || p->tiled_geom_f32 >= kNumGeomF32) return MDSM_OK;
-    if (!build_tables(p, kGeomF32[p->tiled_geom_f32], tt, rs, tab, sig)) return MDSM_OK;
-    if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig)) {
-        mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
-        return MDSM_ECUDA;
+    // rows must be 16-byte aligned for the bulk copies
+    if (p->nsamps % 4 == 0 && p->tiled_geom_f32 >= 0 && p->tiled_geom_f32 < kNumGeomF32) {
+        const int rc = build_one(p, kGeomF32[p->tiled_geom_f32], 4, p->tiled_geom_f32, p->tiled_f32);
+        if (rc != MDSM_OK) return rc;
     }
-    tt.geom = p->tiled_geom_f32;
-    tt.ok = true;
+    if (p->nsamps % 8 == 0 && p->tiled_geom_u8 >= 0 && p->tiled_geom_u8 < kNumGeomU16) {
+        const Geometry &g = kGeomU16[p->tiled_geom_u8];
+        // parts of 256 channels must be whole slabs
+        if (kPartChansU16 % g.CS == 0) {
+            const int rc = build_one(p, g, 8, p->tiled_geom_u8, p->tiled_u8);
+            if (rc != MDSM_OK) return rc;
+        }
+    }
     return MDSM_OK;
 }
 
@@ -435,20 +513,42 @@ void mdsm_tiled_free_tables(mdsm_plan *p)
 {
     free_tables(&p->tiled_f32);
     free_tables(&p->tiled_u8);
+    cudaFree(p->d_widen);
+    p->d_widen = nullptr;
+    p->widen_bytes = 0;
 }
 
 int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
                                  cudaStream_t st)
 {
-    MDSM_REQUIRE(dtype == MDSM_F32, "tiled kernel: only MDSM_F32 so far");
-    const TiledTables &tt = p->tiled_f32;
-    const float *in = (const float *)d_in;
-    float *out = (float *)d_out;
+    if (dtype == MDSM_F32) {
+        const TiledTables &tt = p->tiled_f32;
+        switch (tt.geom) {
+            case 0: return launch_tiled<GeomF32<0>>(p, tt, d_in, beam0, nb, d_out, 0, st);
+            case 1: return launch_tiled<GeomF32<1>>(p, tt, d_in, beam0, nb, d_out, 0, st);
+        }
+        mdsm_set_error("tiled kernel: bad geometry index %d", tt.geom);
+        return MDSM_EINVAL;
+    }
+    // uint8: widen the beams of this call to uint16 in the plan's scratch (allocated on first use, whole plan)
+    const TiledTables &tt = p->tiled_u8;
+    const size_t beam_elems = (size_t)p->nchans * (size_t)p->nsamps;
+    const size_t need = (size_t)p->nbeams * beam_elems * sizeof(uint16_t);
+    if (p->widen_bytes < need) {
+        cudaFree(p->d_widen);
+        p->d_widen = nullptr;
+        p->widen_bytes = 0;
+        MDSM_CUDA_TRY(cudaMalloc(&p->d_widen, need));
+        p->widen_bytes = need;
+    }
+    const uint8_t *src = (const uint8_t *)d_in + (size_t)beam0 * beam_elems;
+    uint16_t *dst = (uint16_t *)p->d_widen + (size_t)beam0 * beam_elems;
+    const size_t n16 = (size_t)nb * beam_elems / 16;
+    widen_u8_kernel<<<p->sm_count * 8, 256, 0, st>>>((const uint4 *)src, (uint4 *)dst, n16);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    p->launches += 1;
     switch (tt.geom) {
-        case 0: return launch_f32<0>(p, tt, in, beam0, nb, out, st);
-        case 1: return launch_f32<1>(p, tt, in, beam0, nb, out, st);
-        case 2: return launch_f32<2>(p, tt, in, beam0, nb, out, st);
-        case 3: return launch_f32<3>(p, tt, in, beam0, nb, out, st);
+        case 0: return launch_tiled<GeomU16<0>>(p, tt, p->d_widen, beam0, nb, d_out, kPartChansU16, st);
     }
     mdsm_set_error("tiled kernel: bad geometry index %d", tt.geom);
     return MDSM_EINVAL;

@@ -1,116 +1,197 @@
 #!/usr/bin/env python
-"""Generates chain_gen.h: the register-window accumulate chains of the tiled dedispersion kernels.
+"""Generates chain_gen.h: the per-slab inner loops of the tiled dedispersion kernels, as inline PTX.
 
-    chain_f32<D,T,NOFF>(acc2[D][T/2], w2[(T+NOFF-1+3)/4*2], o[D]):
-        for j < D:  acc[j][i] += w[o[j] + i],  i < T        (o[j] warp-uniform, 0 <= o[j] < NOFF)
+One call of SlabF32<D,T,NOFF>::run / SlabU16<...>::run processes all channels of one staged slab for
+one warp:
 
-Registers cannot be indexed dynamically, so every (j, offset) pair owns a straight-line block of
-adds.  The blocks are THREADED: block (j, o[j]) ends with the indirect branch (PTX brx.idx -> SASS
-LDC jump-table read + BRX) into block (j+1, o[j+1]), so one channel costs D indirect branches and no
-branch back, and the jump-table read of the next block is issued while the current block's adds run.
-Accumulators and window are packed f32x2 register pairs: an even offset is T/2 FADD2
+    for every channel r of the slab (table entry e_r of this warp):
+        w[0 .. T+NOFF)  <- shared[sbase + e_r.window_start ...]          (128-bit loads)
+        for j < D:  acc[j][i] += w[o_j + i],  i < T                      (o_j = e_r.offset[j], warp-uniform)
+
+Registers cannot be indexed dynamically, so every (j, offset) pair owns a straight-line block of adds and
+the blocks are THREADED: block (j, o_j) ends with the indirect branch (PTX brx.idx -> SASS LDC + BRX) into
+block (j+1, o_{j+1}).  The block of the LAST DM carries a copy of the loop head (next table entry, window
+loads, first dispatch), so one channel costs exactly D taken branches and the whole loop is one asm
+statement -- nvcc wraps nothing in convergence barriers (BSSY/BSYNC/BREAK cost ~70 cycles per channel in the
+r1b profile).
+
+Table entry (64 bit):  lo[17:0]  byte offset of the window start inside the stage
+                       lo[28+i]  load the optional 16-byte chunk T/4 + i   (i = 0, 1, 2)
+                       lo[31]    last channel of the slab for this warp
+                       hi        byte j = register offset o_j of DM j
+
+fp32: accumulators and window are packed f32x2 register pairs; an even offset is T/2 FADD2
 (add.rn.f32x2), an odd offset T scalar FADDs on the halves of the pairs (no register moves).
+u16 : accumulators hold two 16-bit lanes (two consecutive samples) per 32-bit register; the window is kept
+in both phases (we[m] = samples 2m, 2m+1; wo[m] = samples 2m+1, 2m+2, built with one funnel shift per
+register); adds alternate between the ALU pipe (add.u32 -> IADD3) and the FMA pipe (mad.lo.u32 x,1 -> IMAD).
 
-chain_u16<D,T,NOFF> is the integer form: accumulators and window hold two 16-bit lanes per 32-bit
-register (two consecutive samples); an even offset adds the aligned window registers, an odd offset
-the funnel-shifted ones (wo[m] = (w[m] >> 16) | (w[m+1] << 16), built once per channel by the caller).
-
-A C++ `switch` does not work here: nvcc either merges the cases into one add block fed by register
-moves or emits a compare tree.  Run by build.py before nvcc; the output is committed so that the
-repository builds without Python.
+Run by build.py before nvcc; the output is committed so that the repository builds without Python.
 """
 import os
 import sys
 
 
-def wregs(T, NOFF):
-    """window length in 32-bit words: T + NOFF - 1 rounded up to whole 128-bit chunks"""
-    return (T + NOFF - 1 + 3) // 4 * 4
+def nchunks(T, NOFF, per_chunk):
+    """128-bit chunks holding T + NOFF - 1 samples"""
+    return (T + NOFF - 1 + per_chunk - 1) // per_chunk
+
+
+class Emit:
+    def __init__(self):
+        self.lines = []
+
+    def __call__(self, s):
+        self.lines.append(f'        "{s}\\n\\t"')
 
 
 def gen_f32(D, T, NOFF):
-    assert T % 2 == 0
+    assert T % 4 == 0 and D <= 4
     A2 = T // 2
-    W2 = wregs(T, NOFF) // 2
+    NCH = nchunks(T, NOFF, 4)
+    W2 = NCH * 2
+    base_ch = T // 4
+    assert NCH - base_ch <= 3
     nacc = D * A2
-    name = f"chain_f32_{D}_{T}_{NOFF}"
-    s = [f"// f32x2 chain: D={D} DMs x T={T} samples, offsets < {NOFF}"]
-    s.append(f"__device__ __forceinline__ void {name}(unsigned long long (&acc)[{D}][{A2}], const unsigned long long (&w)[{W2}], unsigned lo, unsigned hi)\n{{")
-    s.append('    asm volatile("{\\n\\t"')
-    s.append('        ".reg .f32 a0, a1, x0, x1, y0, y1;\\n\\t"')
-    s.append('        ".reg .b32 ix;\\n\\t"')
+    SB, TAB = nacc, nacc + 1
+    name = f"slab_f32_{D}_{T}_{NOFF}"
+    e = Emit()
+    e("{")
+    e(f".reg .b64 w<{W2}>;")
+    e(".reg .b32 lo, hi, p, tp, ix, tm;")
+    e(".reg .pred q0, q1, q2, pl;")
+    e(".reg .f32 a0, a1, x0, x1, y0, y1;")
     for j in range(D):
-        s.append(f'        "ts{j}: .branchtargets ' + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ';\\n\\t"')
-    LO, HI = nacc + W2, nacc + W2 + 1
+        e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
 
-    def disp(j):
-        # offset of DM j: byte 3 of lo (j = 0), byte j-1 of hi (j >= 1)
-        src, byte = (LO, 3) if j == 0 else (HI, j - 1)
-        return f"prmt.b32 ix, %{src}, 0, 0x444{byte}; brx.idx ix, ts{j};"
+    def head():
+        """decode the entry in (lo, hi), load the window, dispatch DM 0"""
+        e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
+        for i in range(NCH - base_ch):
+            e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
+        e("setp.lt.s32 pl, lo, 0;")
+        for i in range(NCH):
+            pred = f"@q{i - base_ch} " if i >= base_ch else ""
+            e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
+        e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
 
-    s.append(f'        "{disp(0)}\\n\\t"')
+    e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    head()
     for j in range(D):
+        last = j == D - 1
         for k in range(NOFF):
             m = k // 2
+            e(f"B{j}_{k}:")
+            if last:
+                e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")      # next entry (garbage after the last one, unused)
+            else:
+                e(f"prmt.b32 ix, hi, 0, 0x444{j + 1};")
             body = ""
             for i in range(A2):
                 a = j * A2 + i
                 if k % 2 == 0:
-                    body += f"add.rn.f32x2 %{a}, %{a}, %{nacc + m + i}; "
+                    body += f"add.rn.f32x2 %{a}, %{a}, w{m + i}; "
                 else:
-                    body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, %{nacc + m + i}; mov.b64 {{y0,y1}}, %{nacc + m + i + 1}; "
+                    body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, w{m + i}; mov.b64 {{y0,y1}}, w{m + i + 1}; "
                              f"add.f32 a0, a0, x1; add.f32 a1, a1, y0; mov.b64 %{a}, {{a0,a1}}; ")
-            tail = disp(j + 1) if j + 1 < D else "bra.uni Bend;"
-            s.append(f'        "B{j}_{k}: {body}{tail}\\n\\t"')
-    s.append('        "Bend:\\n\\t"')
-    s.append('        "}"')
+            e(body)
+            if last:
+                e("@pl bra.uni Bend;")
+                head()
+            else:
+                e(f"brx.idx ix, ts{j + 1};")
+    e("Bend:")
+    e("}")
+    s = [f"// f32x2 slab loop: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
+    s.append(f"__device__ __forceinline__ void {name}(unsigned long long (&acc)[{D}][{A2}], unsigned sbase, unsigned tab)\n{{")
+    s.append("    asm volatile(")
+    s += e.lines
     s.append("        : " + ", ".join(f'"+l"(acc[{j}][{i}])' for j in range(D) for i in range(A2)))
-    s.append("        : " + ", ".join(f'"l"(w[{i}])' for i in range(W2)) + ', "r"(lo), "r"(hi));')
+    s.append('        : "r"(sbase), "r"(tab) : "memory");')
     s.append("}\n")
-    s.append(f"template <> struct ChainF32<{D}, {T}, {NOFF}> {{ static constexpr int W2 = {W2}; __device__ __forceinline__ static void run(unsigned long long (&a)[{D}][{A2}], const unsigned long long (&w)[{W2}], unsigned lo, unsigned hi) {{ {name}(a, w, lo, hi); }} }};\n")
+    s.append(f"template <> struct SlabF32<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned long long (&a)[{D}][{A2}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
     return "\n".join(s)
 
 
 def gen_u16(D, T, NOFF):
-    """T samples = T/2 registers of two 16-bit lanes.  we[m] = samples (2m, 2m+1); wo[m] = samples (2m+1, 2m+2)."""
-    assert T % 2 == 0
+    """T samples = T/2 registers of two 16-bit lanes; window chunks of 8 samples (16 bytes of u16)."""
+    assert T % 8 == 0 and D <= 4
     A = T // 2
-    WE = wregs(T, NOFF) // 2
-    WO = WE - 1
+    NCH = nchunks(T, NOFF, 8)
+    WE = NCH * 4                      # registers of the even-phase window
+    base_ch = T // 8
+    assert NCH - base_ch <= 3
     nacc = D * A
-    name = f"chain_u16_{D}_{T}_{NOFF}"
-    s = [f"// u16x2 chain: D={D} DMs x T={T} samples, offsets < {NOFF}"]
-    s.append(f"__device__ __forceinline__ void {name}(unsigned (&acc)[{D}][{A}], const unsigned (&we)[{WE}], const unsigned (&wo)[{WO}], const unsigned (&o)[{D}])\n{{")
-    s.append('    asm volatile("{\\n\\t"')
+    SB, TAB = nacc, nacc + 1
+    name = f"slab_u16_{D}_{T}_{NOFF}"
+    e = Emit()
+    e("{")
+    e(f".reg .b32 we<{WE}>, wo<{WE}>;")
+    e(".reg .b32 lo, hi, p, tp, ix, tm;")
+    e(".reg .pred q0, q1, q2, pl;")
     for j in range(D):
-        s.append(f'        "ts{j}: .branchtargets ' + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ';\\n\\t"')
-    s.append(f'        "brx.idx %{nacc + WE + WO}, ts0;\\n\\t"')
+        e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
+
+    def head():
+        e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
+        for i in range(NCH - base_ch):
+            e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
+        e("setp.lt.s32 pl, lo, 0;")
+        for i in range(NCH):
+            pred = f"@q{i - base_ch} " if i >= base_ch else ""
+            e(f"{pred}ld.shared.v4.b32 {{we{4 * i}, we{4 * i + 1}, we{4 * i + 2}, we{4 * i + 3}}}, [p+{16 * i}];")
+        # odd phase: wo[m] = samples (2m+1, 2m+2) = funnel shift of (we[m], we[m+1]) right by 16 bits
+        for m in range(WE - 1):
+            e(f"shf.r.wrap.b32 wo{m}, we{m}, we{m + 1}, 16;")
+        e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+
+    e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    head()
     for j in range(D):
+        last = j == D - 1
         for k in range(NOFF):
             m = k // 2
-            base = nacc + m if k % 2 == 0 else nacc + WE + m
-            body = "".join(f"add.u32 %{j * A + i}, %{j * A + i}, %{base + i}; " for i in range(A))
-            tail = f"brx.idx %{nacc + WE + WO + j + 1}, ts{j + 1};" if j + 1 < D else "bra.uni Bend;"
-            s.append(f'        "B{j}_{k}: {body}{tail}\\n\\t"')
-    s.append('        "Bend:\\n\\t"')
-    s.append('        "}"')
+            src = "we" if k % 2 == 0 else "wo"
+            e(f"B{j}_{k}:")
+            if last:
+                e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
+            else:
+                e(f"prmt.b32 ix, hi, 0, 0x444{j + 1};")
+            body = ""
+            for i in range(A):
+                a = j * A + i
+                if i % 2 == 0:
+                    body += f"add.u32 %{a}, %{a}, {src}{m + i}; "
+                else:
+                    body += f"mad.lo.u32 %{a}, {src}{m + i}, 1, %{a}; "
+            e(body)
+            if last:
+                e("@pl bra.uni Bend;")
+                head()
+            else:
+                e(f"brx.idx ix, ts{j + 1};")
+    e("Bend:")
+    e("}")
+    s = [f"// u16x2 slab loop: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
+    s.append(f"__device__ __forceinline__ void {name}(unsigned (&acc)[{D}][{A}], unsigned sbase, unsigned tab)\n{{")
+    s.append("    asm volatile(")
+    s += e.lines
     s.append("        : " + ", ".join(f'"+r"(acc[{j}][{i}])' for j in range(D) for i in range(A)))
-    s.append("        : " + ", ".join(f'"r"(we[{i}])' for i in range(WE)) + ", " + ", ".join(f'"r"(wo[{i}])' for i in range(WO)) + ", "
-             + ", ".join(f'"r"(o[{j}])' for j in range(D)) + ");")
+    s.append('        : "r"(sbase), "r"(tab) : "memory");')
     s.append("}\n")
-    s.append(f"template <> struct ChainU16<{D}, {T}, {NOFF}> {{ static constexpr int WE = {WE}; __device__ __forceinline__ static void run(unsigned (&a)[{D}][{A}], const unsigned (&we)[{WE}], const unsigned (&wo)[{WO}], const unsigned (&o)[{D}]) {{ {name}(a, we, wo, o); }} }};\n")
+    s.append(f"template <> struct SlabU16<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned (&a)[{D}][{A}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
     return "\n".join(s)
 
 
 # (D, T, NOFF) instances compiled into the library
-F32_VARIANTS = [(4, 28, 12), (4, 20, 12), (5, 20, 16), (4, 28, 16)]
-U16_VARIANTS = []
+F32_VARIANTS = [(4, 28, 12), (4, 20, 12)]
+U16_VARIANTS = [(4, 40, 16)]
 
 
 def main(out):
     parts = ["// GENERATED by gen_chain.py -- do not edit.\n#pragma once\n"]
-    parts.append("template <int D, int T, int NOFF> struct ChainF32;   // packed f32x2 accumulate chain\n")
-    parts.append("template <int D, int T, int NOFF> struct ChainU16;   // packed u16x2 accumulate chain\n")
+    parts.append("template <int D, int T, int NOFF> struct SlabF32;   // packed f32x2 slab loop\n")
+    parts.append("template <int D, int T, int NOFF> struct SlabU16;   // packed u16x2 slab loop\n")
     for v in F32_VARIANTS:
         parts.append(gen_f32(*v))
     for v in U16_VARIANTS:

@@ -29,10 +29,10 @@ void mdsm_set_error(const char *fmt, ...);
 
 // Geometry of the tiled dedispersion kernel (see dedisperse_tiled.cu and DESIGN.md section 6).
 struct TiledTables {
-    int dms_per_warp = 0, warps = 0, tpt = 0;     // D, NW, T (samples per thread)
+    int dms_per_warp = 0, warps = 0, tpt = 0, cs = 0;   // D, NW, T (samples per thread), channels per slab
     int dm_block = 0, n_dm_blocks = 0;            // DB = D*NW
     int tile_t = 0;                               // 32*T output samples per CTA
-    int row_words = 0;                            // staged words per channel row
+    int row_words = 0;                            // staged elements (f32 / u16) per channel row
     int max_off = 0;                              // largest per-DM register offset
     int32_t *d_row_start = nullptr;               // [n_dm_blocks][nchans]   first staged sample - tile_t0
     void *d_warp_tab = nullptr;                   // [n_dm_blocks][nslab][warps][CS] packed window base + per-DM offsets
@@ -63,6 +63,7 @@ struct mdsm_plan {
     int dedisp_kernel = 0;            // 0 auto, 1 direct, 2 tiled
     int tiled_geom_f32 = 0, tiled_geom_u8 = 0;   // compiled tile geometry per dtype (option "tiled_geom")
     TiledTables tiled_f32, tiled_u8;
+    void *d_widen = nullptr; size_t widen_bytes = 0;   // uint16 copy of a uint8 input (allocated on first use)
 
     // host pipeline workspace (allocated on first mdsm_pipeline_host)
     void *ws_in = nullptr; size_t ws_in_bytes = 0;

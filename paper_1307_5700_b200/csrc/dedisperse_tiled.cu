@@ -70,7 +70,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // spinning (a spinning producer warp took 12 % of the SM's issue slots in the r1b profile)
 __device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity)
 {
-    while (!mbar_try_wait(bar, parity)) __nanosleep(256);
+    while (!mbar_try_wait(bar, parity)) __nanosleep(2000);
 }
 __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
 {

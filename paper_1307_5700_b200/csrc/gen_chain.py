@@ -31,6 +31,36 @@ Run by build.py before nvcc; the output is committed so that the repository buil
 import os
 import sys
 
+DEBUG = os.environ.get('MDSM_GEN_DEBUG', '')
+F32_HEAD = os.environ.get('MDSM_GEN_F32_HEAD', 'rep')
+U16_HEAD = os.environ.get('MDSM_GEN_U16_HEAD', 'shared')
+DISPATCH = os.environ.get('MDSM_GEN_DISPATCH', 'tree')     # 'tree' (direct conditional branches) | 'brx' (indirect)
+
+
+def tree_bits(e, j):
+    """predicates b0..b3 <- bits of offset byte j of hi (issued early: they are ready long before the branches)"""
+    for bit in range(4):
+        e(f"and.b32 tm, hi, {1 << (8 * j + bit)}; setp.ne.u32 b{bit}, tm, 0;")
+
+
+def tree_branch(e, j, noff):
+    """branch to B{j}_{o}: at most 4 conditional direct branches, ~2 taken"""
+    def leaf(k):
+        return f"B{j}_{k}" if k < noff else f"B{j}_0"
+    e(f"@b3 bra X{j}_8; @b2 bra X{j}_4; @b1 bra X{j}_2; @b0 bra {leaf(1)}; bra {leaf(0)};")
+
+
+def tree_stubs(e, j, noff):
+    def leaf(k):
+        return f"B{j}_{k}" if k < noff else f"B{j}_0"
+    e(f"X{j}_2: @b0 bra {leaf(3)}; bra {leaf(2)};")
+    e(f"X{j}_4: @b1 bra X{j}_6; @b0 bra {leaf(5)}; bra {leaf(4)};")
+    e(f"X{j}_6: @b0 bra {leaf(7)}; bra {leaf(6)};")
+    e(f"X{j}_8: @b2 bra X{j}_12; @b1 bra X{j}_10; @b0 bra {leaf(9)}; bra {leaf(8)};")
+    e(f"X{j}_10: @b0 bra {leaf(11)}; bra {leaf(10)};")
+    e(f"X{j}_12: @b1 bra X{j}_14; @b0 bra {leaf(13)}; bra {leaf(12)};")
+    e(f"X{j}_14: @b0 bra {leaf(15)}; bra {leaf(14)};")
+
 
 def nchunks(T, NOFF, per_chunk):
     """128-bit chunks holding T + NOFF - 1 samples"""
@@ -59,10 +89,11 @@ def gen_f32(D, T, NOFF):
     e("{")
     e(f".reg .b64 w<{W2}>;")
     e(".reg .b32 lo, hi, p, tp, ix, tm;")
-    e(".reg .pred q0, q1, q2, pl;")
+    e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3;")
     e(".reg .f32 a0, a1, x0, x1, y0, y1;")
-    for j in range(D):
-        e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
+    if DISPATCH == "brx":
+        for j in range(D):
+            e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
 
     def head():
         """decode the entry in (lo, hi), load the window, dispatch DM 0"""
@@ -72,10 +103,16 @@ def gen_f32(D, T, NOFF):
         e("setp.lt.s32 pl, lo, 0;")
         for i in range(NCH):
             pred = f"@q{i - base_ch} " if i >= base_ch else ""
-            e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
-        e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+            if DEBUG != "nolds" or i == 0:
+                e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
+        if DISPATCH == "brx":
+            e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+        else:
+            tree_bits(e, 0)
+            tree_branch(e, 0, NOFF)
 
     e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    e("HEAD:")
     head()
     for j in range(D):
         last = j == D - 1
@@ -84,8 +121,10 @@ def gen_f32(D, T, NOFF):
             e(f"B{j}_{k}:")
             if last:
                 e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")      # next entry (garbage after the last one, unused)
-            else:
+            elif DISPATCH == "brx":
                 e(f"prmt.b32 ix, hi, 0, 0x444{j + 1};")
+            else:
+                tree_bits(e, j + 1)
             body = ""
             for i in range(A2):
                 a = j * A2 + i
@@ -94,12 +133,22 @@ def gen_f32(D, T, NOFF):
                 else:
                     body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, w{m + i}; mov.b64 {{y0,y1}}, w{m + i + 1}; "
                              f"add.f32 a0, a0, x1; add.f32 a1, a1, y0; mov.b64 %{a}, {{a0,a1}}; ")
+            if DEBUG == "noadd":
+                body = f"add.rn.f32x2 %{j * A2}, %{j * A2}, w{m}; "
             e(body)
             if last:
                 e("@pl bra.uni Bend;")
-                head()
-            else:
+                if F32_HEAD == "shared":
+                    e("bra.uni HEAD;")
+                else:
+                    head()
+            elif DISPATCH == "brx":
                 e(f"brx.idx ix, ts{j + 1};")
+            else:
+                tree_branch(e, j + 1, NOFF)
+    if DISPATCH != "brx":
+        for j in range(D):
+            tree_stubs(e, j, NOFF)
     e("Bend:")
     e("}")
     s = [f"// f32x2 slab loop: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
@@ -128,9 +177,10 @@ def gen_u16(D, T, NOFF):
     e("{")
     e(f".reg .b32 we<{WE}>, wo<{WE}>;")
     e(".reg .b32 lo, hi, p, tp, ix, tm;")
-    e(".reg .pred q0, q1, q2, pl;")
-    for j in range(D):
-        e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
+    e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3;")
+    if DISPATCH == "brx":
+        for j in range(D):
+            e(f"ts{j}: .branchtargets " + ", ".join(f"B{j}_{k}" for k in range(NOFF)) + ";")
 
     def head():
         e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
@@ -143,9 +193,14 @@ def gen_u16(D, T, NOFF):
         # odd phase: wo[m] = samples (2m+1, 2m+2) = funnel shift of (we[m], we[m+1]) right by 16 bits
         for m in range(WE - 1):
             e(f"shf.r.wrap.b32 wo{m}, we{m}, we{m + 1}, 16;")
-        e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+        if DISPATCH == "brx":
+            e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+        else:
+            tree_bits(e, 0)
+            tree_branch(e, 0, NOFF)
 
     e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    e("HEAD:")
     head()
     for j in range(D):
         last = j == D - 1
@@ -155,8 +210,10 @@ def gen_u16(D, T, NOFF):
             e(f"B{j}_{k}:")
             if last:
                 e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
-            else:
+            elif DISPATCH == "brx":
                 e(f"prmt.b32 ix, hi, 0, 0x444{j + 1};")
+            else:
+                tree_bits(e, j + 1)
             body = ""
             for i in range(A):
                 a = j * A + i
@@ -167,9 +224,17 @@ def gen_u16(D, T, NOFF):
             e(body)
             if last:
                 e("@pl bra.uni Bend;")
-                head()
-            else:
+                if U16_HEAD == "shared":
+                    e("bra.uni HEAD;")        # the u16 head (window loads + funnel shifts) is too long to copy 16 times
+                else:
+                    head()
+            elif DISPATCH == "brx":
                 e(f"brx.idx ix, ts{j + 1};")
+            else:
+                tree_branch(e, j + 1, NOFF)
+    if DISPATCH != "brx":
+        for j in range(D):
+            tree_stubs(e, j, NOFF)
     e("Bend:")
     e("}")
     s = [f"// u16x2 slab loop: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]

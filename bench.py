@@ -25,6 +25,17 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 NOMINAL_ADD_PEAK = 148 * 128 * 1.965e9          # SMs x FP32/INT32 lanes x max SM clock (B200_PROFILING.md)
+# DRAM bytes of one dedispersion launch from the committed ncu captures (profiles/r1e_*.md); null for other configs
+NCU_TRAFFIC_BYTES = {"cfg3-8beam-f32": 4.04e9, "cfg4-8beam-u8": 3.92e9}
+
+
+def measured_hbm_peak() -> float:
+    """HBM bytes/s from the driver-written MEASURED_PEAKS.json, else the profiling guide's fallback figure."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]) * 1e9
+    except Exception:
+        return 6.65e12          # B200_PROFILING.md fallback
 
 
 class ClockSampler:
@@ -79,6 +90,24 @@ class ClockSampler:
                     pass
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """Max of a per-rank number over the process group (the contract's "max over ranks"); identity at world 1."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(units_per_rank: float, world: int, ms_per_step_rank: float, device=None):
+    """Whole-job value: every rank processes its own `units_per_rank` per step (beam sharding, no exchange step),
+    the step time is the slowest rank's.  Returns (value, ms_per_step)."""
+    ms = max_over_ranks(ms_per_step_rank, world, device)
+    return units_per_rank * world / (ms * 1e-3), ms
 
 
 def oracle_chain_sample(cfg, x_beam):
@@ -218,14 +247,8 @@ def main():
     dd_ms = [e[1].elapsed_time(e[2]) for e in evs]
     det_ms = [e[2].elapsed_time(e[3]) for e in evs]
     chain_ms = [e[0].elapsed_time(e[3]) for e in evs]
-    chain_total = sum(chain_ms)
-    if world > 1:
-        tt = torch.tensor([chain_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        chain_total = float(tt.item())
-    ms_per_step = chain_total / args.steps
+    value, ms_per_step = job_throughput(cfg.nbeams * cfg.ndms * nso, world, sum(chain_ms) / args.steps, "cuda")
     units_per_step = cfg.nbeams * cfg.ndms * nso * world
-    value = units_per_step / (ms_per_step * 1e-3)
 
     # ---- end to end through the host-buffer C-ABI call (H2D of the input and D2H of the events inside) ----
     e2e = None
@@ -243,10 +266,7 @@ def main():
                                              max_events, args.nstreams)
         barrier()
         te = (time.perf_counter() - te) / n_e2e
-        if world > 1:
-            tt = torch.tensor([te], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            te = float(tt.item())
+        te = max_over_ranks(te, world, "cuda")
         launches_e2e = (m.mdsm_plan_launch_count(plan) - l1) // n_e2e
         e2e = {"value": units_per_step / te, "unit": "DM-trial samples/s", "h2d_bytes_per_step": int(x.nbytes),
                "d2h_bytes_per_step": int(cnt_h * 16 + 8), "ms_per_step": 1e3 * te, "events": cnt_h,
@@ -258,10 +278,12 @@ def main():
     dd = statistics.mean(dd_ms) * 1e-3
     adds = float(cfg.nchans) * cfg.nbeams * cfg.ndms * nso          # algorithmic adds per launch
     hbm_bytes = x.nbytes + 4.0 * cfg.nbeams * cfg.ndms * nso
+    hbm_peak = measured_hbm_peak()
     roofline = {"bound": "alu", "kernel": "dedisperse", "achieved": adds / dd / 1e9, "peak": peak / 1e9, "unit": "Gadd/s",
                 "frac": adds / dd / peak, "peak_source": "measured in this run: mdsm_measure_add_peak (register-only add loop, all SMs)",
                 "peak_nominal": NOMINAL_ADD_PEAK / 1e9, "measured_peaks_gadd_s": {k: v / 1e9 for k, v in peaks.items()},
-                "ms_per_launch": dd * 1e3, "hbm_floor_ms": 1e3 * hbm_bytes / 6.551e12, "traffic": None}
+                "ms_per_launch": dd * 1e3, "hbm_floor_ms": 1e3 * hbm_bytes / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full capture under profiles/ (r1e)"}
 
     line = {
         "metric": "DM-trial samples/s", "value": value, "unit": "DM-trial samples/s", "n_gpus": world,

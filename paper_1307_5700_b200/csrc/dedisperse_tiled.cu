@@ -27,7 +27,6 @@
 // boundaries, so a CTA never drains its pipeline between tiles.
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <vector>
 
 #include "chain_gen.h"
@@ -149,14 +148,14 @@ struct TiledArgs {
 };
 
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
-    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, NOFF = NOFF_, AW = T_ / 2;
+    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
     static constexpr bool kF32 = true;
     using In = float; using Out = float; using Acc = unsigned long long;
     using Slab = SlabF32<D_, T_, NOFF_>;
     static_assert(T_ % 4 == 0 && (T_ / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
 };
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
-    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, NOFF = NOFF_, AW = T_ / 2;
+    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
     static constexpr bool kF32 = false;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16<D_, T_, NOFF_>;
@@ -405,8 +404,7 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, TiledTab
                 for (int i = 0; i < extra; ++i) lo |= 1ULL << (28 + i);
                 if (last) lo |= 1ULL << 31;
                 unsigned long long hi = 0;
-                static const char *dbg_force = getenv("MDSM_DEBUG_FORCE_OFFSET");   // experiments only: wrong results
-                for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(dbg_force ? atoi(dbg_force) : (e[j] - A)) << (8 * j);
+                for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(e[j] - A) << (8 * j);
                 h_tab[(((size_t)blk * nslab + slab) * g.NW + w) * g.CS + r] = lo | (hi << 32);
             }
         }
@@ -444,13 +442,11 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
     if (stages > 12) stages = 12;
     MDSM_REQUIRE(stages >= 2, "tiled kernel: staged rows too large for shared memory");
     const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t) + 16;
-    int cur = 0;
     static thread_local size_t smem_set = 0;
     if (smem > smem_set) {
         MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         smem_set = smem;
     }
-    (void)cur;
     TiledArgs a;
     a.in = d_in; a.out = d_out;
     a.row_start = tt.d_row_start; a.warp_tab = (const unsigned long long *)tt.d_warp_tab; a.sigma = tt.d_sigma;

@@ -31,8 +31,8 @@ Run by build.py before nvcc; the output is committed so that the repository buil
 import os
 import sys
 
-DEBUG = os.environ.get('MDSM_GEN_DEBUG', '')
 F32_HEAD = os.environ.get('MDSM_GEN_F32_HEAD', 'rep')
+U16_DISPATCH = os.environ.get('MDSM_GEN_U16_DISPATCH', 'shared')
 U16_HEAD = os.environ.get('MDSM_GEN_U16_HEAD', 'shared')
 DISPATCH = os.environ.get('MDSM_GEN_DISPATCH', 'tree')     # 'tree' (direct conditional branches) | 'brx' (indirect)
 
@@ -103,8 +103,7 @@ def gen_f32(D, T, NOFF):
         e("setp.lt.s32 pl, lo, 0;")
         for i in range(NCH):
             pred = f"@q{i - base_ch} " if i >= base_ch else ""
-            if DEBUG != "nolds" or i == 0:
-                e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
+            e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
         if DISPATCH == "brx":
             e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
         else:
@@ -133,8 +132,6 @@ def gen_f32(D, T, NOFF):
                 else:
                     body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, w{m + i}; mov.b64 {{y0,y1}}, w{m + i + 1}; "
                              f"add.f32 a0, a0, x1; add.f32 a1, a1, y0; mov.b64 %{a}, {{a0,a1}}; ")
-            if DEBUG == "noadd":
-                body = f"add.rn.f32x2 %{j * A2}, %{j * A2}, w{m}; "
             e(body)
             if last:
                 e("@pl bra.uni Bend;")
@@ -195,6 +192,8 @@ def gen_u16(D, T, NOFF):
             e(f"shf.r.wrap.b32 wo{m}, we{m}, we{m + 1}, 16;")
         if DISPATCH == "brx":
             e("prmt.b32 ix, hi, 0, 0x4440; brx.idx ix, ts0;")
+        elif U16_DISPATCH == "shared":
+            e("bra.uni DISP0;")
         else:
             tree_bits(e, 0)
             tree_branch(e, 0, NOFF)
@@ -212,7 +211,7 @@ def gen_u16(D, T, NOFF):
                 e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
             elif DISPATCH == "brx":
                 e(f"prmt.b32 ix, hi, 0, 0x444{j + 1};")
-            else:
+            elif U16_DISPATCH != "shared":
                 tree_bits(e, j + 1)
             body = ""
             for i in range(A):
@@ -230,10 +229,16 @@ def gen_u16(D, T, NOFF):
                     head()
             elif DISPATCH == "brx":
                 e(f"brx.idx ix, ts{j + 1};")
+            elif U16_DISPATCH == "shared":
+                e(f"bra.uni DISP{j + 1};")
             else:
                 tree_branch(e, j + 1, NOFF)
     if DISPATCH != "brx":
         for j in range(D):
+            if U16_DISPATCH == "shared":      # one dispatcher per DM slot keeps the hot code inside the L1.5 I-cache
+                e(f"DISP{j}:")
+                tree_bits(e, j)
+                tree_branch(e, j, NOFF)
             tree_stubs(e, j, NOFF)
     e("Bend:")
     e("}")

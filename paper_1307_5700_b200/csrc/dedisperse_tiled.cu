@@ -149,16 +149,26 @@ struct TiledArgs {
 
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
-    static constexpr bool kF32 = true;
+    static constexpr bool kF32 = true, kTwoPhase = false;
     using In = float; using Out = float; using Acc = unsigned long long;
     using Slab = SlabF32<D_, T_, NOFF_>;
     static_assert(T_ % 4 == 0 && (T_ / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
 };
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
-    static constexpr bool kF32 = false;
+    static constexpr bool kF32 = false, kTwoPhase = false;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16<D_, T_, NOFF_>;
+    static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
+};
+
+// two-phase integer variant: per DM an even-phase row E (T/2 registers) and an odd-phase row O (T/2 + 1 registers,
+// outputs shifted by one sample), no shifted window copy (gen_chain.py: gen_u16p)
+template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16P {
+    static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ + 1;
+    static constexpr bool kF32 = false, kTwoPhase = true;
+    using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
+    using Slab = SlabU16P<D_, T_, NOFF_>;
     static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
 };
 
@@ -268,8 +278,11 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
                 if (d >= a.ndms) continue;
                 Out v[T];
 #pragma unroll
-                for (int i = 0; i < AW; ++i) {
-                    if constexpr (Tr::kF32) {
+                for (int i = 0; i < T / 2; ++i) {
+                    if constexpr (Tr::kTwoPhase) {
+                        v[2 * i] = (acc[j][i] & 0xffffu) + (acc[j][T / 2 + i] >> 16);
+                        v[2 * i + 1] = (acc[j][i] >> 16) + (acc[j][T / 2 + i + 1] & 0xffffu);
+                    } else if constexpr (Tr::kF32) {
                         v[2 * i] = __uint_as_float((unsigned)acc[j][i]);
                         v[2 * i + 1] = __uint_as_float((unsigned)(acc[j][i] >> 32));
                     } else {
@@ -286,18 +299,16 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
     }
 }
 
-// widens the uint8 filterbank to uint16 (the staged element type of the integer kernel)
-__global__ void __launch_bounds__(256) widen_u8_kernel(const uint4 *__restrict__ in, uint4 *__restrict__ out, size_t n16)
+// widens the uint8 filterbank to uint16 (the staged element type of the integer kernels), 8 samples per thread and
+// step (nsamps % 8 == 0 is a condition of the tiled integer path, so every beam is a whole number of such groups)
+__global__ void __launch_bounds__(256) widen_u8_kernel(const uint2 *__restrict__ in, uint4 *__restrict__ out, size_t n8)
 {
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) {
-        const uint4 v = in[i];
-        uint4 a, b;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        const uint2 v = in[i];
+        uint4 a;
         a.x = __byte_perm(v.x, 0, 0x4140); a.y = __byte_perm(v.x, 0, 0x4342);
         a.z = __byte_perm(v.y, 0, 0x4140); a.w = __byte_perm(v.y, 0, 0x4342);
-        b.x = __byte_perm(v.z, 0, 0x4140); b.y = __byte_perm(v.z, 0, 0x4342);
-        b.z = __byte_perm(v.w, 0, 0x4140); b.w = __byte_perm(v.w, 0, 0x4342);
-        out[2 * i] = a;
-        out[2 * i + 1] = b;
+        out[i] = a;
     }
 }
 
@@ -307,7 +318,7 @@ struct Geometry {
 };
 // compiled geometries; index = plan option "tiled_geom_<dtype>"
 constexpr Geometry kGeomF32[] = {{4, 28, 11, 8, 12}, {4, 20, 15, 8, 12}};
-constexpr Geometry kGeomU16[] = {{4, 40, 11, 8, 16}};
+constexpr Geometry kGeomU16[] = {{2, 40, 15, 8, 12}, {3, 40, 11, 8, 14}, {4, 40, 11, 8, 16}};   // index <= 1: two-phase rows
 constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
 constexpr int kNumGeomU16 = sizeof(kGeomU16) / sizeof(kGeomU16[0]);
 constexpr int kPartChansU16 = 256;          // 256 * 255 < 2^16: the most channels a 16-bit lane can take
@@ -317,7 +328,7 @@ static inline long long floor_to(long long v, int a) { return v >= 0 ? (v / a) *
 // Builds the row-start / per-warp window tables for one geometry.  `al` = samples per 16 bytes of the staged
 // element type.  Returns false if this plan's delay spread does not fit the geometry's register window (the
 // caller then uses the direct kernel).
-static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, TiledTables &tt, std::vector<int32_t> &h_rs,
+static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, bool two_phase, TiledTables &tt, std::vector<int32_t> &h_rs,
                          std::vector<unsigned long long> &h_tab, std::vector<int32_t> &h_sigma)
 {
     const int DB = g.D * g.NW, TT = 32 * g.T;
@@ -404,7 +415,10 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, TiledTab
                 for (int i = 0; i < extra; ++i) lo |= 1ULL << (28 + i);
                 if (last) lo |= 1ULL << 31;
                 unsigned long long hi = 0;
-                for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(e[j] - A) << (8 * j);
+                for (int j = 0; j < g.D; ++j) {
+                    const unsigned long long o = (unsigned long long)(e[j] - A);
+                    hi |= (two_phase ? 8 * (o & 1) + (o >> 1) : o) << (8 * j);      // dispatch index of DM j
+                }
                 h_tab[(((size_t)blk * nslab + slab) * g.NW + w) * g.CS + r] = lo | (hi << 32);
             }
         }
@@ -466,12 +480,13 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
 
 template <int G> using GeomF32 = TraitsF32<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
 template <int G> using GeomU16 = TraitsU16<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
+template <int G> using GeomU16P = TraitsU16P<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
 
-static int build_one(mdsm_plan *p, const Geometry &g, int al, int geom, TiledTables &tt)
+static int build_one(mdsm_plan *p, const Geometry &g, int al, bool two_phase, int geom, TiledTables &tt)
 {
     std::vector<int32_t> rs, sig;
     std::vector<unsigned long long> tab;
-    if (!build_tables(p, g, al, tt, rs, tab, sig)) return MDSM_OK;
+    if (!build_tables(p, g, al, two_phase, tt, rs, tab, sig)) return MDSM_OK;
     if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig)) {
         mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         return MDSM_ECUDA;
@@ -491,14 +506,14 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
     free_tables(&p->tiled_u8);
     // rows must be 16-byte aligned for the bulk copies
     if (p->nsamps % 4 == 0 && p->tiled_geom_f32 >= 0 && p->tiled_geom_f32 < kNumGeomF32) {
-        const int rc = build_one(p, kGeomF32[p->tiled_geom_f32], 4, p->tiled_geom_f32, p->tiled_f32);
+        const int rc = build_one(p, kGeomF32[p->tiled_geom_f32], 4, false, p->tiled_geom_f32, p->tiled_f32);
         if (rc != MDSM_OK) return rc;
     }
     if (p->nsamps % 8 == 0 && p->tiled_geom_u8 >= 0 && p->tiled_geom_u8 < kNumGeomU16) {
         const Geometry &g = kGeomU16[p->tiled_geom_u8];
         // parts of 256 channels must be whole slabs
         if (kPartChansU16 % g.CS == 0) {
-            const int rc = build_one(p, g, 8, p->tiled_geom_u8, p->tiled_u8);
+            const int rc = build_one(p, g, 8, p->tiled_geom_u8 <= 1, p->tiled_geom_u8, p->tiled_u8);
             if (rc != MDSM_OK) return rc;
         }
     }
@@ -539,12 +554,14 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
     }
     const uint8_t *src = (const uint8_t *)d_in + (size_t)beam0 * beam_elems;
     uint16_t *dst = (uint16_t *)p->d_widen + (size_t)beam0 * beam_elems;
-    const size_t n16 = (size_t)nb * beam_elems / 16;
-    widen_u8_kernel<<<p->sm_count * 8, 256, 0, st>>>((const uint4 *)src, (uint4 *)dst, n16);
+    const size_t n8 = (size_t)nb * beam_elems / 8;
+    widen_u8_kernel<<<p->sm_count * 8, 256, 0, st>>>((const uint2 *)src, (uint4 *)dst, n8);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 1;
     switch (tt.geom) {
-        case 0: return launch_tiled<GeomU16<0>>(p, tt, p->d_widen, beam0, nb, d_out, kPartChansU16, st);
+        case 0: return launch_tiled<GeomU16P<0>>(p, tt, p->d_widen, beam0, nb, d_out, kPartChansU16, st);
+        case 1: return launch_tiled<GeomU16P<1>>(p, tt, p->d_widen, beam0, nb, d_out, kPartChansU16, st);
+        case 2: return launch_tiled<GeomU16<2>>(p, tt, p->d_widen, beam0, nb, d_out, kPartChansU16, st);
     }
     mdsm_set_error("tiled kernel: bad geometry index %d", tt.geom);
     return MDSM_EINVAL;

@@ -253,19 +253,99 @@ def gen_u16(D, T, NOFF):
     return "\n".join(s)
 
 
+def gen_u16p(D, T, NOFF):
+    """Two-phase u16x2 loop: no shifted window.  Every DM keeps TWO accumulator rows:
+         E[i] = outputs (2i, 2i+1), i < T/2      fed by channels whose offset o = 2m is even:  E[i] += we[m+i]
+         O[i] = outputs (2i-1, 2i), i <= T/2     fed by channels whose offset o = 2m+1 is odd: O[i] += we[m+i]
+       (the outer halves of O[0] and O[T/2] belong to the neighbouring threads and are dropped); the epilogue adds
+       the two rows.  Dispatch index = 8*(o & 1) + (o >> 1)."""
+    assert T % 8 == 0 and D <= 4 and NOFF <= 16
+    A = T // 2
+    AW = 2 * A + 1
+    NCH = nchunks(T, NOFF, 8)
+    WE = NCH * 4
+    base_ch = T // 8
+    assert NCH - base_ch <= 3
+    nacc = D * AW
+    SB, TAB = nacc, nacc + 1
+    name = f"slab_u16p_{D}_{T}_{NOFF}"
+    e = Emit()
+    e("{")
+    e(f".reg .b32 we<{WE}>;")
+    e(".reg .b32 lo, hi, p, tp, tm;")
+    e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3;")
+
+    def head():
+        e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
+        for i in range(NCH - base_ch):
+            e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
+        e("setp.lt.s32 pl, lo, 0;")
+        for i in range(NCH):
+            pred = f"@q{i - base_ch} " if i >= base_ch else ""
+            e(f"{pred}ld.shared.v4.b32 {{we{4 * i}, we{4 * i + 1}, we{4 * i + 2}, we{4 * i + 3}}}, [p+{16 * i}];")
+        tree_bits(e, 0)
+        tree_branch(e, 0, 16)
+
+    e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    head()
+    for j in range(D):
+        last = j == D - 1
+        for idx in range(16):
+            odd, m = idx // 8, idx % 8
+            e(f"B{j}_{idx}:")
+            if 2 * m + odd >= NOFF:                 # unreachable index: keep the label, no code
+                e("bra.uni Bend;")
+                continue
+            if last:
+                e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
+            else:
+                tree_bits(e, j + 1)
+            body = ""
+            n = A + 1 if odd else A
+            for i in range(n):
+                a = j * AW + (A + i if odd else i)
+                if i % 2 == 0:
+                    body += f"add.u32 %{a}, %{a}, we{m + i}; "
+                else:
+                    body += f"mad.lo.u32 %{a}, we{m + i}, 1, %{a}; "
+            e(body)
+            if last:
+                e("@pl bra.uni Bend;")
+                head()
+            else:
+                tree_branch(e, j + 1, 16)
+    for j in range(D):
+        tree_stubs(e, j, 16)
+    e("Bend:")
+    e("}")
+    s = [f"// two-phase u16x2 slab loop: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
+    s.append(f"__device__ __forceinline__ void {name}(unsigned (&acc)[{D}][{AW}], unsigned sbase, unsigned tab)\n{{")
+    s.append("    asm volatile(")
+    s += e.lines
+    s.append("        : " + ", ".join(f'"+r"(acc[{j}][{i}])' for j in range(D) for i in range(AW)))
+    s.append('        : "r"(sbase), "r"(tab) : "memory");')
+    s.append("}\n")
+    s.append(f"template <> struct SlabU16P<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned (&a)[{D}][{AW}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
+    return "\n".join(s)
+
+
 # (D, T, NOFF) instances compiled into the library
 F32_VARIANTS = [(4, 28, 12), (4, 20, 12)]
 U16_VARIANTS = [(4, 40, 16)]
+U16P_VARIANTS = [(2, 40, 12), (3, 40, 14)]
 
 
 def main(out):
     parts = ["// GENERATED by gen_chain.py -- do not edit.\n#pragma once\n"]
     parts.append("template <int D, int T, int NOFF> struct SlabF32;   // packed f32x2 slab loop\n")
     parts.append("template <int D, int T, int NOFF> struct SlabU16;   // packed u16x2 slab loop\n")
+    parts.append("template <int D, int T, int NOFF> struct SlabU16P;  // two-phase packed u16x2 slab loop\n")
     for v in F32_VARIANTS:
         parts.append(gen_f32(*v))
     for v in U16_VARIANTS:
         parts.append(gen_u16(*v))
+    for v in U16P_VARIANTS:
+        parts.append(gen_u16p(*v))
     txt = "\n".join(parts)
     if os.path.exists(out) and open(out).read() == txt:
         return

@@ -30,6 +30,8 @@ SHAPES = {
     "one_dm": (1, 16, 418.0, -1.0, 51.2e-6, 2048, 3.0, 0.0, 1),
     "one_chan": (2, 1, 418.0, -1.0, 51.2e-6, 1024, 0.0, 0.5, 9),
     "wide": (1, 512, 418.0, -20.0 / 512, 51.2e-6, 16384, 0.0, 0.1, 200),
+    "tail8": (3, 37, 418.0, -0.5, 51.2e-6, 5000, 0.0, 0.13, 13),            # beams of 8k (not 16k) samples: u16 widening tail
+    "parts": (2, 300, 418.0, -20.0 / 300, 51.2e-6, 16384, 0.0, 0.1, 100),   # two 256-channel parts on the integer path
 }
 
 

@@ -180,6 +180,7 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
     using Out = typename Tr::Out;
     using Acc = typename Tr::Acc;
     constexpr int D = Tr::D, T = Tr::T, NW = Tr::NW, CS = Tr::CS, AW = Tr::AW, DB = D * NW;
+    static_assert(CS <= 31, "producer lanes 0..CS-1 copy rows, lane CS the table slice");
     extern __shared__ __align__(128) unsigned char smem[];
     const int stages = a.stages;
     const uint32_t stage_bytes = (uint32_t)CS * a.row_elems * sizeof(In);
@@ -317,8 +318,8 @@ struct Geometry {
     int D, T, NW, CS, NOFF;
 };
 // compiled geometries; index = plan option "tiled_geom_<dtype>"
-constexpr Geometry kGeomF32[] = {{4, 28, 11, 8, 12}, {4, 20, 15, 8, 12}};
-constexpr Geometry kGeomU16[] = {{2, 40, 15, 8, 12}, {3, 40, 11, 8, 14}, {4, 40, 11, 8, 16}};   // index <= 1: two-phase rows
+constexpr Geometry kGeomF32[] = {{4, 28, 11, 16, 12}, {4, 20, 15, 8, 12}};
+constexpr Geometry kGeomU16[] = {{2, 40, 15, 16, 12}, {3, 40, 11, 8, 14}, {4, 40, 11, 8, 16}};   // index <= 1: two-phase rows
 constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
 constexpr int kNumGeomU16 = sizeof(kGeomU16) / sizeof(kGeomU16[0]);
 constexpr int kPartChansU16 = 256;          // 256 * 255 < 2^16: the most channels a 16-bit lane can take

@@ -47,19 +47,19 @@ def tree_branch(e, j, noff):
     """branch to B{j}_{o}: at most 4 conditional direct branches, ~2 taken"""
     def leaf(k):
         return f"B{j}_{k}" if k < noff else f"B{j}_0"
-    e(f"@b3 bra X{j}_8; @b2 bra X{j}_4; @b1 bra X{j}_2; @b0 bra {leaf(1)}; bra {leaf(0)};")
+    e(f"@b3 bra.uni X{j}_8; @b2 bra.uni X{j}_4; @b1 bra.uni X{j}_2; @b0 bra.uni {leaf(1)}; bra.uni {leaf(0)};")
 
 
 def tree_stubs(e, j, noff):
     def leaf(k):
         return f"B{j}_{k}" if k < noff else f"B{j}_0"
-    e(f"X{j}_2: @b0 bra {leaf(3)}; bra {leaf(2)};")
-    e(f"X{j}_4: @b1 bra X{j}_6; @b0 bra {leaf(5)}; bra {leaf(4)};")
-    e(f"X{j}_6: @b0 bra {leaf(7)}; bra {leaf(6)};")
-    e(f"X{j}_8: @b2 bra X{j}_12; @b1 bra X{j}_10; @b0 bra {leaf(9)}; bra {leaf(8)};")
-    e(f"X{j}_10: @b0 bra {leaf(11)}; bra {leaf(10)};")
-    e(f"X{j}_12: @b1 bra X{j}_14; @b0 bra {leaf(13)}; bra {leaf(12)};")
-    e(f"X{j}_14: @b0 bra {leaf(15)}; bra {leaf(14)};")
+    e(f"X{j}_2: @b0 bra.uni {leaf(3)}; bra.uni {leaf(2)};")
+    e(f"X{j}_4: @b1 bra.uni X{j}_6; @b0 bra.uni {leaf(5)}; bra.uni {leaf(4)};")
+    e(f"X{j}_6: @b0 bra.uni {leaf(7)}; bra.uni {leaf(6)};")
+    e(f"X{j}_8: @b2 bra.uni X{j}_12; @b1 bra.uni X{j}_10; @b0 bra.uni {leaf(9)}; bra.uni {leaf(8)};")
+    e(f"X{j}_10: @b0 bra.uni {leaf(11)}; bra.uni {leaf(10)};")
+    e(f"X{j}_12: @b1 bra.uni X{j}_14; @b0 bra.uni {leaf(13)}; bra.uni {leaf(12)};")
+    e(f"X{j}_14: @b0 bra.uni {leaf(15)}; bra.uni {leaf(14)};")
 
 
 def nchunks(T, NOFF, per_chunk):

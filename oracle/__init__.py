@@ -161,3 +161,24 @@ def detect(series: np.ndarray, n_valid: int, snr_thresh: float, max_events: int 
     ev = ev[: min(cnt, max_events)]
     ev = ev[np.lexsort((ev["t"], ev["dm_idx"], ev["beam"]))]
     return ev, int(cnt), stats
+
+
+def median_filter(series: np.ndarray, n_valid: int, window: int) -> np.ndarray:
+    """Windowed median of every series[..., :n_valid] (Eq. 2; reading E-i); the tail is copied."""
+    assert series.dtype == np.float32 and series.flags.c_contiguous and window >= 1 and window % 2 == 1 and window <= 1023
+    stride = series.shape[-1]
+    out = series.copy()
+    _L().orc_median_filter_f32(_p(series), c_int64(series.size // stride), c_int64(stride), c_int64(n_valid), c_int(window), _p(out))
+    return out
+
+
+def detrend(series: np.ndarray, n_valid: int):
+    """Subtract the least-squares line and divide by the residual's standard deviation (reading E-ii).
+    Returns (normalised float32 array, params[..., 3] = mean, slope, std)."""
+    assert series.dtype == np.float32 and series.flags.c_contiguous
+    stride = series.shape[-1]
+    ns = series.size // stride
+    out = series.copy()
+    params = np.empty(series.shape[:-1] + (3,), dtype=np.float64)
+    _L().orc_detrend_f32(_p(series), c_int64(ns), c_int64(stride), c_int64(n_valid), _p(out), _p(params))
+    return out, params

@@ -368,3 +368,73 @@ int64_t orc_detect_u32(const uint32_t *series, int64_t nseries, int ndms, int64_
 {
     ORC_DETECT_BODY(uint32_t, 1)
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Post-processing of the dedispersed series (section 2.2.3) -- SURVEY 8(f) NEXT-1.
+ *
+ * orc_median_filter_f32: Eq. 2 with operation = median: y[m] = median{ x[i], i in w }, w = the
+ *   neighbourhood of `window` (odd) points centred on m.  Readings (E-i): the neighbourhood is
+ *   clipped to the valid samples [0, n) at the two ends (the paper's kernel loads "overlapping values at the edges"
+ *   but does not say what stands in beyond the series); with an even number of points left, the median is the mean
+ *   of the two middle ones.  Pinned by brute force against numpy.median and by isolated-outlier / monotone-series
+ *   invariants (tests/test_oracle_postprocess.py).
+ * orc_detrend_f32: best-fit line by linear regression over t = 0..n-1 (pass 1), subtract it and take the standard
+ *   deviation of the residual (pass 2), divide (pass 3) -- PAPER.md:110.  Population standard deviation (1/n);
+ *   a series with zero residual variance becomes all zeros (reading E-ii).  fp64 throughout, result cast to float.
+ *   Pinned against the closed-form least-squares solution (numpy.polyfit) and exact lines.
+ * ------------------------------------------------------------------------------------------------ */
+void orc_median_filter_f32(const float *in, int64_t nseries, int64_t stride, int64_t n, int window, float *out)
+{
+    const int h = window / 2;
+#pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < nseries; ++s) {
+        const float *x = in + s * stride;
+        float *y = out + s * stride;
+        float buf[1024];
+        for (int64_t m = 0; m < n; ++m) {
+            int64_t lo = m - h, hi = m + h;
+            if (lo < 0) lo = 0;
+            if (hi > n - 1) hi = n - 1;
+            int cnt = 0;
+            for (int64_t i = lo; i <= hi; ++i) {          /* insertion sort of the neighbourhood */
+                float v = x[i];
+                int k = cnt++;
+                while (k > 0 && buf[k - 1] > v) { buf[k] = buf[k - 1]; --k; }
+                buf[k] = v;
+            }
+            if (cnt & 1) y[m] = buf[cnt / 2];
+            else y[m] = (float)(((double)buf[cnt / 2 - 1] + (double)buf[cnt / 2]) / 2.0);
+        }
+    }
+}
+
+/* params[s] = (mean, slope, std of the residual) */
+void orc_detrend_f32(const float *in, int64_t nseries, int64_t stride, int64_t n, float *out, double *params)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < nseries; ++s) {
+        const float *x = in + s * stride;
+        float *y = out + s * stride;
+        const double tbar = ((double)n - 1.0) / 2.0;
+        double sy = 0.0, sty = 0.0, stt = 0.0;
+        for (int64_t t = 0; t < n; ++t) {                /* pass 1: regression parameters */
+            const double dt = (double)t - tbar;
+            sy += (double)x[t];
+            sty += dt * (double)x[t];
+            stt += dt * dt;
+        }
+        const double mean = sy / (double)n;
+        const double slope = stt > 0.0 ? sty / stt : 0.0;
+        double sr = 0.0;
+        for (int64_t t = 0; t < n; ++t) {                /* pass 2: residual variance */
+            const double r = (double)x[t] - (mean + slope * ((double)t - tbar));
+            sr += r * r;
+        }
+        const double sd = sqrt(sr / (double)n);
+        for (int64_t t = 0; t < n; ++t) {                /* pass 3: normalise */
+            const double r = (double)x[t] - (mean + slope * ((double)t - tbar));
+            y[t] = sd > 0.0 ? (float)(r / sd) : 0.0f;
+        }
+        if (params) { params[3 * s] = mean; params[3 * s + 1] = slope; params[3 * s + 2] = sd; }
+    }
+}

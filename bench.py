@@ -169,6 +169,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--nstreams", type=int, default=4)
+    ap.add_argument("--postprocess", type=int, default=0,
+                    help="median window W: also time mdsm_median_filter(W) + mdsm_detrend on the dedispersed series (fp32 "
+                         "configs; reported beside the chain, not part of `value`)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -251,6 +254,29 @@ def main():
     value, ms_per_step = job_throughput(cfg.nbeams * cfg.ndms * nso, world, sum(chain_ms) / args.steps, "cuda")
     units_per_step = cfg.nbeams * cfg.ndms * nso * world
 
+    # ---- optional: the paper's post-processing stage, timed on the series of the last step ----
+    post = None
+    if args.postprocess and cfg.dtype == "f32":
+        filt = torch.empty_like(out)
+        pe = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        tm, td = [], []
+        for _ in range(max(3, min(args.steps, 10))):
+            work.copy_(pristine)                                   # L2 flush between repetitions
+            pe[0].record(stream)
+            m.mdsm_median_filter(plan, out, filt, 0, cfg.nbeams, args.postprocess, stream)
+            pe[1].record(stream)
+            m.mdsm_detrend(plan, filt, 0, cfg.nbeams, None, stream)
+            pe[2].record(stream)
+            torch.cuda.synchronize()
+            tm.append(pe[0].elapsed_time(pe[1])); td.append(pe[1].elapsed_time(pe[2]))
+        sbytes = 4.0 * cfg.nbeams * cfg.ndms * nso
+        hp = measured_hbm_peak()
+        post = {"median_window": args.postprocess, "median_ms": statistics.mean(tm), "detrend_ms": statistics.mean(td),
+                "median_hbm_frac": 2 * sbytes / (statistics.mean(tm) * 1e-3) / hp,
+                "detrend_hbm_frac": 2 * sbytes / (statistics.mean(td) * 1e-3) / hp,
+                "algorithmic_bytes": "one read + one write of the valid series per kernel"}
+        del filt
+
     # ---- end to end through the host-buffer C-ABI call (H2D of the input and D2H of the events inside) ----
     e2e = None
     if not args.no_e2e:
@@ -300,6 +326,8 @@ def main():
         "events_per_step": n_events, "gpu_launches": int(launches), "clocks": clocks,
         "e2e": e2e, "roofline": roofline,
     }
+    if post:
+        line["postprocess"] = post
 
     if rank == 0 and not args.no_cpu_baseline and world >= 1:
         import oracle

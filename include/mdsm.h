@@ -97,6 +97,22 @@ int mdsm_detect(mdsm_plan *plan, const void *d_out, int dtype, int beam0, int nb
                 double snr_thresh, mdsm_event *d_events, int64_t max_events,
                 unsigned long long *d_count, void *cuda_stream);
 
+/* Post-processing of the dedispersed series between mdsm_dedisperse and mdsm_detect (section
+ * 2.2.3: "optional post-processing").  fp32 series only, layout of d_out ([nbeams][ndms][nsamps], the
+ * first nsamps_out samples of a row valid); device pointers, asynchronous on cuda_stream, no allocation.
+ *
+ * mdsm_median_filter: Eq. 2 with operation = median, y[m] = median{x[i], i in w}, w = `window`
+ *   (odd, <= 33) samples centred on m, clipped to the valid samples at the two ends; an even number of remaining
+ *   points gives the mean of the two middle ones.  d_filtered must be a different buffer of the same layout; only
+ *   t < nsamps_out of the rows [beam0, beam0+nb) is written.
+ * mdsm_detrend: per series, subtract the least-squares line over t = 0..nsamps_out-1 and divide by the population
+ *   standard deviation of the residual, in place; a series with zero residual variance becomes
+ *   zeros.  d_params (may be NULL) receives [nbeams][ndms][3] = mean, slope, standard deviation (fp64, device).
+ * Errors: MDSM_EINVAL for a bad beam range / window / null or aliased buffers. */
+int mdsm_median_filter(mdsm_plan *plan, const float *d_series, float *d_filtered, int beam0, int nb, int window,
+                       void *cuda_stream);
+int mdsm_detrend(mdsm_plan *plan, float *d_series, int beam0, int nb, double *d_params, void *cuda_stream);
+
 /* The whole chain from HOST buffers (per-beam threads copy their input to the GPU;
  * north_star item 4: beam groups on separate CUDA streams with overlapped host-to-device copies).
  * h_in [nbeams][nchans][nsamps] (pinned memory overlaps best); the clipped data is NOT copied back.

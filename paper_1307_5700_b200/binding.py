@@ -17,7 +17,7 @@ __all__ = [
     "EVENT_DTYPE", "MdsmError", "lib_path",
     "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
-    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_pipeline_host", "mdsm_measure_add_peak",
+    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_pipeline_host", "mdsm_measure_add_peak",
 ]
 
 MDSM_F32, MDSM_U8 = 0, 1
@@ -67,6 +67,10 @@ def _load():
     L.mdsm_dedisperse.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
     L.mdsm_detect.restype = c_int
     L.mdsm_detect.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_double, c_void_p, c_int64, c_void_p, c_void_p]
+    L.mdsm_median_filter.restype = c_int
+    L.mdsm_median_filter.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_void_p]
+    L.mdsm_detrend.restype = c_int
+    L.mdsm_detrend.argtypes = [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p]
     L.mdsm_pipeline_host.restype = c_int
     L.mdsm_pipeline_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, c_double, c_void_p,
                                      c_int64, POINTER(c_uint64), c_int]
@@ -167,6 +171,14 @@ def mdsm_dedisperse(plan, d_in, beam0, nb, d_out, stream=None, dtype=None) -> No
 def mdsm_detect(plan, d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, stream=None, dtype=None) -> None:
     _check(_L.mdsm_detect(plan, _ptr(d_out), _dtype_of(d_out, dtype), beam0, nb, snr_thresh, _ptr(d_events),
                           max_events, _ptr(d_count), _stream(stream)))
+
+
+def mdsm_median_filter(plan, d_series, d_filtered, beam0, nb, window, stream=None) -> None:
+    _check(_L.mdsm_median_filter(plan, _ptr(d_series), _ptr(d_filtered), beam0, nb, window, _stream(stream)))
+
+
+def mdsm_detrend(plan, d_series, beam0, nb, d_params=None, stream=None) -> None:
+    _check(_L.mdsm_detrend(plan, _ptr(d_series), beam0, nb, _ptr(d_params), _stream(stream)))
 
 
 def mdsm_pipeline_host(plan, h_in, window, k_chan, k_spec, snr_thresh, h_events, max_events, nstreams=4,

@@ -5,8 +5,10 @@
 //                        reduction (uint64 exact for uint32 series, fp64 for float series),
 //                        then mean / rms with single IEEE fp64 ops in the oracle's order.
 //   threshold_emit_kernel  every sample: snr = ((double)x - mean)/rms > thr ?  Candidates are
-//                        pre-filtered with one fp64 subtract-compare; events are appended with
-//                        warp-aggregated atomics (one atomicAdd per warp per vote).
+//                        pre-filtered in the element type (one compare per sample against a bound
+//                        rounded down; a warp without candidates leaves), then with one fp64
+//                        subtract-compare; events are appended with warp-aggregated atomics (one
+//                        atomicAdd per warp per vote).
 #include "mdsm_internal.h"
 
 namespace {
@@ -23,6 +25,9 @@ template <typename A> __device__ __forceinline__ A wsum(A v)
 template <typename T> __device__ __forceinline__ T as_elem(unsigned w);
 template <> __device__ __forceinline__ float as_elem<float>(unsigned w) { return __uint_as_float(w); }
 template <> __device__ __forceinline__ uint32_t as_elem<uint32_t>(unsigned w) { return w; }
+
+template <typename T> constexpr bool kIsFloat = false;
+template <> constexpr bool kIsFloat<float> = true;
 
 template <typename T> struct SAcc;
 template <> struct SAcc<float> { using type = double; };
@@ -107,6 +112,26 @@ threshold_emit_kernel(const T *__restrict__ out, int beam0, int ndms, long long 
         for (int k = 0; k < 4; ++k) v[k] = (t0 + k < n) ? x[t0 + k] : (T)0;
     }
     const int lane = threadIdx.x & 31;
+    // Cheap conservative pre-filter in the element type: a sample can only be an event if x > mean + cut, so one
+    // compare per sample against a bound rounded DOWN (with a 1e-12 relative margin for the fp64 subtraction below)
+    // rules almost everything out, and a warp none of whose 128 samples passes skips the fp64 path altogether.
+    bool cand = false;
+    {
+        const double bound = mean + cut;
+        const double slack = bound - (fabs(bound) * 1e-12 + 1e-300);
+        if (kIsFloat<T>) {                                         // float series
+            const float cf = __double2float_rd(slack);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) cand |= (t0 + k < n) && ((float)v[k] > cf);
+        } else {                                                    // uint32 series
+            const double fl = floor(slack);
+            const bool all = fl < 0.0;
+            const uint32_t cu = all ? 0u : (fl >= 4294967295.0 ? 0xffffffffu : (uint32_t)fl);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) cand |= (t0 + k < n) && (all || (uint32_t)v[k] > cu);
+        }
+    }
+    if (!__any_sync(0xffffffffu, cand)) return;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         bool hit = false;

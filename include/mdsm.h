@@ -58,7 +58,9 @@ int mdsm_plan_get_delays(const mdsm_plan *plan, int32_t *h_delays);
 const char *mdsm_last_error(void);
 
 /* Plan options.  key "dedisp_kernel": 0 = auto, 1 = direct (global-load reference kernel),
- * 2 = tiled (shared-memory staged, register-blocked).  Unknown key/value -> MDSM_EINVAL. */
+ * 2 = tiled (shared-memory staged, register-blocked).  key "tiled_geom_f32" / "tiled_geom_u8": index of the compiled
+ * tile geometry, -1 (default) = the first one whose register window takes the plan's delay spread; if none does, or
+ * rows are not 16-byte aligned, the direct kernel runs.  Unknown key/value -> MDSM_EINVAL. */
 int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);
 /* Number of kernels this plan has launched since creation (all entry points). */
 int64_t mdsm_plan_launch_count(const mdsm_plan *plan);

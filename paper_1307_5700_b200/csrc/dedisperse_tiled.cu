@@ -318,7 +318,7 @@ struct Geometry {
     int D, T, NW, CS, NOFF;
 };
 // compiled geometries; index = plan option "tiled_geom_<dtype>"
-constexpr Geometry kGeomF32[] = {{4, 28, 11, 16, 12}, {4, 20, 15, 8, 12}};
+constexpr Geometry kGeomF32[] = {{4, 28, 11, 16, 12}, {4, 20, 15, 8, 12}, {2, 28, 15, 16, 12}};   // last: coarse DM grids
 constexpr Geometry kGeomU16[] = {{2, 40, 15, 16, 12}, {3, 40, 11, 8, 14}, {4, 40, 11, 8, 16}};   // index <= 1: two-phase rows
 constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
 constexpr int kNumGeomU16 = sizeof(kGeomU16) / sizeof(kGeomU16[0]);
@@ -505,19 +505,21 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
 {
     free_tables(&p->tiled_f32);
     free_tables(&p->tiled_u8);
-    // rows must be 16-byte aligned for the bulk copies
-    if (p->nsamps % 4 == 0 && p->tiled_geom_f32 >= 0 && p->tiled_geom_f32 < kNumGeomF32) {
-        const int rc = build_one(p, kGeomF32[p->tiled_geom_f32], 4, false, p->tiled_geom_f32, p->tiled_f32);
-        if (rc != MDSM_OK) return rc;
-    }
-    if (p->nsamps % 8 == 0 && p->tiled_geom_u8 >= 0 && p->tiled_geom_u8 < kNumGeomU16) {
-        const Geometry &g = kGeomU16[p->tiled_geom_u8];
-        // parts of 256 channels must be whole slabs
-        if (kPartChansU16 % g.CS == 0) {
-            const int rc = build_one(p, g, 8, p->tiled_geom_u8 <= 1, p->tiled_geom_u8, p->tiled_u8);
+    // Rows must be 16-byte aligned for the bulk copies.  tiled_geom_* < 0 = automatic: the first compiled geometry
+    // whose register window takes this plan's delay spread (coarser DM grids need fewer DMs per warp).
+    if (p->nsamps % 4 == 0 && p->tiled_geom_f32 < kNumGeomF32)
+        for (int g = 0; g < kNumGeomF32 && !p->tiled_f32.ok; ++g) {
+            if (p->tiled_geom_f32 >= 0 && g != p->tiled_geom_f32) continue;
+            const int rc = build_one(p, kGeomF32[g], 4, false, g, p->tiled_f32);
             if (rc != MDSM_OK) return rc;
         }
-    }
+    if (p->nsamps % 8 == 0 && p->tiled_geom_u8 < kNumGeomU16)
+        for (int g = 0; g < kNumGeomU16 && !p->tiled_u8.ok; ++g) {
+            if (p->tiled_geom_u8 >= 0 && g != p->tiled_geom_u8) continue;
+            if (kPartChansU16 % kGeomU16[g].CS != 0) continue;       // parts of 256 channels must be whole slabs
+            const int rc = build_one(p, kGeomU16[g], 8, g <= 1, g, p->tiled_u8);
+            if (rc != MDSM_OK) return rc;
+        }
     return MDSM_OK;
 }
 
@@ -538,6 +540,7 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
         switch (tt.geom) {
             case 0: return launch_tiled<GeomF32<0>>(p, tt, d_in, beam0, nb, d_out, 0, st);
             case 1: return launch_tiled<GeomF32<1>>(p, tt, d_in, beam0, nb, d_out, 0, st);
+            case 2: return launch_tiled<GeomF32<2>>(p, tt, d_in, beam0, nb, d_out, 0, st);
         }
         mdsm_set_error("tiled kernel: bad geometry index %d", tt.geom);
         return MDSM_EINVAL;

@@ -330,7 +330,7 @@ def gen_u16p(D, T, NOFF):
 
 
 # (D, T, NOFF) instances compiled into the library
-F32_VARIANTS = [(4, 28, 12), (4, 20, 12)]
+F32_VARIANTS = [(4, 28, 12), (4, 20, 12), (2, 28, 12)]
 U16_VARIANTS = [(4, 40, 16)]
 U16P_VARIANTS = [(2, 40, 12), (3, 40, 14)]
 

@@ -61,7 +61,7 @@ struct mdsm_plan {
     double *d_series_stats = nullptr; // [nbeams][ndms][2] = mean, rms
 
     int dedisp_kernel = 0;            // 0 auto, 1 direct, 2 tiled
-    int tiled_geom_f32 = 0, tiled_geom_u8 = 0;   // compiled tile geometry per dtype (option "tiled_geom")
+    int tiled_geom_f32 = -1, tiled_geom_u8 = -1;   // compiled tile geometry per dtype (option "tiled_geom_*"), -1 = automatic
     TiledTables tiled_f32, tiled_u8;
     void *d_widen = nullptr; size_t widen_bytes = 0;   // uint16 copy of a uint8 input (allocated on first use)
 

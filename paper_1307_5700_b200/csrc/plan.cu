@@ -159,7 +159,7 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
     }
     if (strcmp(key, "tiled_geom_f32") == 0 || strcmp(key, "tiled_geom_u8") == 0) {
         const bool f = key[11] == 'f';
-        MDSM_REQUIRE(value >= 0 && value < mdsm_tiled_num_geoms(f ? MDSM_F32 : MDSM_U8), "no such tile geometry");
+        MDSM_REQUIRE(value >= -1 && value < mdsm_tiled_num_geoms(f ? MDSM_F32 : MDSM_U8), "no such tile geometry (-1 = automatic)");
         (f ? p->tiled_geom_f32 : p->tiled_geom_u8) = (int)value;
         return mdsm_tiled_build_tables(p);
     }

@@ -90,3 +90,21 @@ def test_no_events_constant_input_and_argument_errors():
                 (0, 8, 418.0, -0.5, 51.2e-6, 1024, 0.0, 0.1, 4)):
         with pytest.raises(m.MdsmError):
             m.mdsm_plan_create(*bad)
+
+
+def test_coarse_dm_grid_selects_a_narrower_tile_geometry():
+    """dm_step = 0.3: three times the delay spread per DM step of the BEST-2 grid.  The automatic geometry choice must
+    still find a tiled fp32 kernel (fewer DMs per warp); whatever runs must match the oracle."""
+    torch = _torch()
+    args = (2, 256, 418.0, -20.0 / 256, 51.2e-6, 16384, 0.0, 0.3, 60)
+    g = np.random.default_rng(8)
+    d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
+    xf = g.normal(size=(2, 256, 16384)).astype(np.float32)
+    xu = g.integers(0, 256, size=(2, 256, 16384)).astype(np.uint8)
+    with Plan(args) as p:
+        ref, ab = oracle.dedisperse(xf, d)
+        got = out_to_numpy(p.dedisperse(torch.from_numpy(xf).cuda(), kernel=2), p.nsamps_out)      # tiled, not direct
+        assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)
+        refu, _ = oracle.dedisperse(xu, d)
+        gotu = out_to_numpy(p.dedisperse(torch.from_numpy(xu).cuda(), kernel=0), p.nsamps_out)
+        assert np.array_equal(gotu, refu)

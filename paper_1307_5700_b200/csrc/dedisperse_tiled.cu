@@ -13,11 +13,12 @@
 // from shared memory with conflict-free 128-bit loads and adds it, at D different register offsets, into
 // its D accumulator rows -- every shared-memory word feeds ~3 adds, which is what lifts the kernel off the
 // 32 words/clk/SM shared-memory ceiling (25 % of the add peak).  The offsets are warp-uniform; they select
-// straight-line add blocks through a threaded chain of indirect branches (chain_gen.h, gen_chain.py).
+// straight-line add blocks, chained through short trees of direct conditional branches (chain_gen.h, gen_chain.py).
 //   fp32: accumulators and window are packed f32x2 register pairs (FADD2 for even offsets).
 //   u8  : the input is widened once to u16 (plan scratch); accumulators are packed u16x2 lanes (one add =
 //         two samples), flushed into the uint32 output after every part (part 0 stores, later parts
-//         read-modify-write their own elements, which are still in L2).
+//         read-modify-write their own elements, which are still in L2).  Every DM keeps an even-phase and an
+//         odd-phase accumulator row, so that odd register offsets need no shifted copy of the window.
 // The time axis is SHEARED: DM d of a block owns outputs [tile_t0 - sigma_d, tile_t0 - sigma_d + 32T)
 // with sigma_d ~ half the band-edge delay slope, which halves the spread of the D windows (and of the
 // staged rows) compared with an unsheared tile.

@@ -9,11 +9,13 @@ one warp:
         for j < D:  acc[j][i] += w[o_j + i],  i < T                      (o_j = e_r.offset[j], warp-uniform)
 
 Registers cannot be indexed dynamically, so every (j, offset) pair owns a straight-line block of adds and
-the blocks are THREADED: block (j, o_j) ends with the indirect branch (PTX brx.idx -> SASS LDC + BRX) into
-block (j+1, o_{j+1}).  The block of the LAST DM carries a copy of the loop head (next table entry, window
-loads, first dispatch), so one channel costs exactly D taken branches and the whole loop is one asm
-statement -- nvcc wraps nothing in convergence barriers (BSSY/BSYNC/BREAK cost ~70 cycles per channel in the
-r1b profile).
+the blocks are THREADED: block (j, o_j) ends by branching into block (j+1, o_{j+1}).  The dispatch is a short
+tree of DIRECT predicated branches on the bits of o_{j+1} (predicates computed at the top of the block, ~2 taken
+branches); the PTX `brx.idx` form (SASS LDC jump-table read + BRX; MDSM_GEN_DISPATCH=brx) cost ~90 instead of
+~35 warp-cycles per dispatch.  The block of the LAST DM carries a copy of the loop head (next table entry,
+window loads, first dispatch) and the whole loop is one asm statement -- nvcc wraps nothing in convergence
+barriers (BSSY/BSYNC/BREAK cost ~70 cycles per channel in the r1b profile).  The hot code has to stay inside
+the 32 KB L1.5 instruction cache: the integer kernels share one loop head instead of copying it.
 
 Table entry (64 bit):  lo[17:0]  byte offset of the window start inside the stage
                        lo[28+i]  load the optional 16-byte chunk T/4 + i   (i = 0, 1, 2)
@@ -22,9 +24,9 @@ Table entry (64 bit):  lo[17:0]  byte offset of the window start inside the stag
 
 fp32: accumulators and window are packed f32x2 register pairs; an even offset is T/2 FADD2
 (add.rn.f32x2), an odd offset T scalar FADDs on the halves of the pairs (no register moves).
-u16 : accumulators hold two 16-bit lanes (two consecutive samples) per 32-bit register; the window is kept
-in both phases (we[m] = samples 2m, 2m+1; wo[m] = samples 2m+1, 2m+2, built with one funnel shift per
-register); adds alternate between the ALU pipe (add.u32 -> IADD3) and the FMA pipe (mad.lo.u32 x,1 -> IMAD).
+u16 : accumulators hold two 16-bit lanes (two consecutive samples) per 32-bit register.  gen_u16 keeps the window
+in both phases (we[m] = samples 2m, 2m+1; wo[m] = samples 2m+1, 2m+2, one funnel shift per register); gen_u16p
+(the default) keeps two accumulator rows per DM instead (even / odd offsets) and adds the window as loaded.
 
 Run by build.py before nvcc; the output is committed so that the repository builds without Python.
 """

@@ -168,7 +168,7 @@ def main():
     ap.add_argument("--geom", type=int, default=-1, help="tiled_geom_<dtype> option (compiled tile geometry); -1 = plan default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--nstreams", type=int, default=4)
+    ap.add_argument("--nstreams", type=int, default=8)
     ap.add_argument("--postprocess", type=int, default=0,
                     help="median window W: also time mdsm_median_filter(W) + mdsm_detrend on the dedispersed series (fp32 "
                          "configs; reported beside the chain, not part of `value`)")

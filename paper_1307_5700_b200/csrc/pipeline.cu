@@ -1,7 +1,7 @@
 // Host-buffer chain: multibeam batching across CUDA streams with overlapped host-to-device
 // copies (BASELINE.json north_star item 4; the paper's per-beam threads each copy their own
-// beam to the GPU).  Beam b runs on stream b % nstreams:
-//   H2D(beam b) -> clip -> dedisperse -> detect, so beam b+1's copy overlaps beam b's compute.
+// beam to the GPU).  The beams are split into nstreams contiguous groups, group g on stream g:
+//   H2D(group g) -> clip -> dedisperse -> detect, so group g+1's copy overlaps group g's compute.
 #include "mdsm_internal.h"
 
 static int ensure(void **ptr, size_t *have, size_t need)
@@ -55,13 +55,17 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
     MDSM_CUDA_TRY(cudaEventRecord(p->ws_done[0], p->ws_streams[0]));
     for (int s = 1; s < nstreams; ++s) MDSM_CUDA_TRY(cudaStreamWaitEvent(p->ws_streams[s], p->ws_done[0], 0));
 
-    for (int b = 0; b < p->nbeams; ++b) {
-        cudaStream_t st = p->ws_streams[b % nstreams];
-        MDSM_CUDA_TRY(cudaMemcpyAsync((char *)p->ws_in + beam_in * b, (const char *)h_in + beam_in * b, beam_in,
+    // contiguous beam groups, one per stream: whole groups per launch keep the persistent dedispersion grid full
+    // (one beam is only ~7 waves of tiles), while group g+1's copy still overlaps group g's kernels
+    const int per = (p->nbeams + nstreams - 1) / nstreams;
+    for (int b = 0, g = 0; b < p->nbeams; b += per, ++g) {
+        cudaStream_t st = p->ws_streams[g % nstreams];
+        const int nb = b + per <= p->nbeams ? per : p->nbeams - b;
+        MDSM_CUDA_TRY(cudaMemcpyAsync((char *)p->ws_in + beam_in * b, (const char *)h_in + beam_in * b, beam_in * nb,
                                       cudaMemcpyHostToDevice, st));
-        if (window > 0 && (rc = mdsm_rfi_clip(p, p->ws_in, dtype, b, 1, window, k_chan, k_spec, nullptr, nullptr, st))) return rc;
-        if ((rc = mdsm_dedisperse(p, p->ws_in, dtype, b, 1, p->ws_out, st))) return rc;
-        if ((rc = mdsm_detect(p, p->ws_out, dtype, b, 1, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
+        if (window > 0 && (rc = mdsm_rfi_clip(p, p->ws_in, dtype, b, nb, window, k_chan, k_spec, nullptr, nullptr, st))) return rc;
+        if ((rc = mdsm_dedisperse(p, p->ws_in, dtype, b, nb, p->ws_out, st))) return rc;
+        if ((rc = mdsm_detect(p, p->ws_out, dtype, b, nb, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
     }
     // join every stream into stream 0, then read back the count and the events
     for (int s = 1; s < nstreams; ++s) {

@@ -68,6 +68,8 @@ struct mdsm_plan {
     // host pipeline workspace (allocated on first mdsm_pipeline_host)
     void *ws_in = nullptr; size_t ws_in_bytes = 0;
     void *ws_out = nullptr; size_t ws_out_bytes = 0;
+    void *ws_filt = nullptr; size_t ws_filt_bytes = 0;    // median-filtered series (options post_median_window)
+    int post_median_window = 0, post_detrend = 0;         // optional post-processing inside mdsm_pipeline_host (fp32)
     mdsm_event *ws_events = nullptr; int64_t ws_max_events = 0;
     unsigned long long *ws_count = nullptr;
     std::vector<cudaStream_t> ws_streams;

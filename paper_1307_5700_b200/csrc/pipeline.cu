@@ -35,6 +35,9 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
     int rc;
     if ((rc = ensure(&p->ws_in, &p->ws_in_bytes, beam_in * p->nbeams))) return rc;
     if ((rc = ensure(&p->ws_out, &p->ws_out_bytes, (size_t)p->nbeams * p->ndms * p->nsamps * 4))) return rc;
+    const bool post = dtype == MDSM_F32 && (p->post_median_window > 1 || p->post_detrend);
+    if (post && p->post_median_window > 1 &&
+        (rc = ensure(&p->ws_filt, &p->ws_filt_bytes, (size_t)p->nbeams * p->ndms * p->nsamps * 4))) return rc;
     if (!p->ws_events || p->ws_max_events < max_events) {
         cudaFree(p->ws_events);
         p->ws_events = nullptr;
@@ -65,7 +68,15 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
                                       cudaMemcpyHostToDevice, st));
         if (window > 0 && (rc = mdsm_rfi_clip(p, p->ws_in, dtype, b, nb, window, k_chan, k_spec, nullptr, nullptr, st))) return rc;
         if ((rc = mdsm_dedisperse(p, p->ws_in, dtype, b, nb, p->ws_out, st))) return rc;
-        if ((rc = mdsm_detect(p, p->ws_out, dtype, b, nb, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
+        const void *series = p->ws_out;
+        if (post) {                      // the paper's optional post-processing stage, fp32 series only
+            if (p->post_median_window > 1) {
+                if ((rc = mdsm_median_filter(p, (const float *)p->ws_out, (float *)p->ws_filt, b, nb, p->post_median_window, st))) return rc;
+                series = p->ws_filt;
+            }
+            if (p->post_detrend && (rc = mdsm_detrend(p, (float *)series, b, nb, nullptr, st))) return rc;
+        }
+        if ((rc = mdsm_detect(p, series, dtype, b, nb, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
     }
     // join every stream into stream 0, then read back the count and the events
     for (int s = 1; s < nstreams; ++s) {

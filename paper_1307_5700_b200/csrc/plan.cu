@@ -128,6 +128,7 @@ extern "C" void mdsm_plan_destroy(mdsm_plan *p)
     cudaFree(p->d_spec_part);
     cudaFree(p->d_spec_part_u);
     cudaFree(p->d_series_stats);
+    cudaFree(p->ws_filt);
     mdsm_tiled_free_tables(p);
     cudaFree(p->ws_in);
     cudaFree(p->ws_out);
@@ -155,6 +156,16 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
     if (strcmp(key, "dedisp_kernel") == 0) {
         MDSM_REQUIRE(value >= 0 && value <= 2, "dedisp_kernel must be 0 (auto), 1 (direct) or 2 (tiled)");
         p->dedisp_kernel = (int)value;
+        return MDSM_OK;
+    }
+    if (strcmp(key, "post_median_window") == 0) {
+        MDSM_REQUIRE(value == 0 || (value >= 1 && value <= 33 && (value & 1)), "post_median_window must be 0 (off) or odd and <= 33");
+        p->post_median_window = (int)value;
+        return MDSM_OK;
+    }
+    if (strcmp(key, "post_detrend") == 0) {
+        MDSM_REQUIRE(value == 0 || value == 1, "post_detrend must be 0 or 1");
+        p->post_detrend = (int)value;
         return MDSM_OK;
     }
     if (strcmp(key, "tiled_geom_f32") == 0 || strcmp(key, "tiled_geom_u8") == 0) {

@@ -101,3 +101,27 @@ def test_chain_with_postprocess_cfg1():
         assert compare_events_f32(ev_g, ev_o, cfg.snr_thresh) > 0
         top = ev_g[np.argmax(ev_g["snr"])]
         assert top["dm_idx"] == 20 and 999 <= top["t"] <= 1004   # the 4-sample pulse survives a 5-point median
+
+
+def test_pipeline_host_with_postprocess_options():
+    """mdsm_pipeline_host with plan options post_median_window / post_detrend = the same events as the separate calls."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    cfg = CONFIGS[1]
+    x = generate(cfg)
+    with Plan(cfg) as p:
+        out = p.dedisperse(torch.from_numpy(x).cuda())
+        filt = torch.zeros_like(out)
+        m.mdsm_median_filter(p.h, out, filt, 0, 1, 5)
+        m.mdsm_detrend(p.h, filt, 0, 1, None)
+        ev_sep, cnt_sep = p.detect(filt, cfg.snr_thresh)
+        m.mdsm_plan_set_option(p.h, "post_median_window", 5)
+        m.mdsm_plan_set_option(p.h, "post_detrend", 1)
+        hev = np.zeros(4096, dtype=m.EVENT_DTYPE)
+        rc, cnt = m.mdsm_pipeline_host(p.h, x, 0, 0.0, 0.0, cfg.snr_thresh, hev, 4096, 1)       # window 0: no clip
+        assert rc == m.MDSM_OK and cnt == cnt_sep > 0
+        hev = hev[:cnt]
+        hev = hev[np.lexsort((hev["t"], hev["dm_idx"], hev["beam"]))]
+        assert np.array_equal(hev, ev_sep)
+        with pytest.raises(m.MdsmError):
+            m.mdsm_plan_set_option(p.h, "post_median_window", 4)

@@ -182,3 +182,11 @@ def detrend(series: np.ndarray, n_valid: int):
     params = np.empty(series.shape[:-1] + (3,), dtype=np.float64)
     _L().orc_detrend_f32(_p(series), c_int64(ns), c_int64(stride), c_int64(n_valid), _p(out), _p(params))
     return out, params
+
+
+def power_i16(volt: np.ndarray) -> np.ndarray:
+    """|re + i im|^2 of interleaved int16 voltages [..., 2] -> float32 [...]."""
+    assert volt.dtype == np.int16 and volt.shape[-1] == 2 and volt.flags.c_contiguous
+    out = np.empty(volt.shape[:-1], dtype=np.float32)
+    _L().orc_power_i16(_p(volt), c_int64(out.size), _p(out))
+    return out

@@ -438,3 +438,18 @@ void orc_detrend_f32(const float *in, int64_t nseries, int64_t stride, int64_t n
         if (params) { params[3 * s] = mean; params[3 * s + 1] = slope; params[3 * s + 2] = sd; }
     }
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Power calculation (the first GPU stage, "power calculation", on the 16-bit complex channelised
+ * voltages of the beamformer) -- SURVEY 8(f) NEXT-4.
+ *   power[i] = re[i]^2 + im[i]^2, voltages interleaved (re, im) int16; the sum is an exact integer < 2^31 + 1, the
+ *   result is that integer rounded to nearest float.  Pinned by hand-computed values (tests/test_oracle_power.py).
+ * ------------------------------------------------------------------------------------------------ */
+void orc_power_i16(const int16_t *volt, int64_t n, float *power)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        const int64_t re = volt[2 * i], im = volt[2 * i + 1];
+        power[i] = (float)(double)(re * re + im * im);      /* int64 -> double exact, double -> float round to nearest */
+    }
+}

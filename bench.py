@@ -276,6 +276,20 @@ def main():
                 "detrend_hbm_frac": 2 * sbytes / (statistics.mean(td) * 1e-3) / hp,
                 "algorithmic_bytes": "one read + one write of the valid series per kernel"}
         del filt
+        # the paper's first GPU stage (power from 16-bit complex voltages, NEXT-4) on a buffer of the input's shape
+        nel = cfg.nbeams * cfg.nchans * cfg.nsamps
+        volt = torch.randint(-2048, 2048, (nel, 2), dtype=torch.int16, device="cuda")
+        tp = []
+        for _ in range(5):
+            out.zero_()                                            # 1.3 GB write: flushes L2
+            pe[0].record(stream)
+            m.mdsm_power_i16(volt, work, nel, stream)
+            pe[1].record(stream)
+            torch.cuda.synchronize()
+            tp.append(pe[0].elapsed_time(pe[1]))
+        post["power_ms"] = statistics.mean(tp[1:])
+        post["power_hbm_frac"] = 8.0 * nel / (post["power_ms"] * 1e-3) / hp
+        del volt
 
     # ---- end to end through the host-buffer C-ABI call (H2D of the input and D2H of the events inside) ----
     e2e = None

@@ -117,6 +117,13 @@ int mdsm_median_filter(mdsm_plan *plan, const float *d_series, float *d_filtered
                        void *cuda_stream);
 int mdsm_detrend(mdsm_plan *plan, float *d_series, int beam0, int nb, double *d_params, void *cuda_stream);
 
+/* Power calculation, the first GPU stage of the paper's pipeline: d_power[i] = re^2 + im^2 of the
+ * 16-bit complex channelised voltages d_volt[i] = (re, im), any layout (the call is element-wise, so
+ * [beam][chan][time][2] in gives [beam][chan][time] out).  The sum is exact in integers and rounded once to float.
+ * Device pointers, 16-byte aligned, caller-owned; asynchronous on cuda_stream; needs no plan.  MDSM_EINVAL for
+ * null / misaligned buffers or n < 0. */
+int mdsm_power_i16(const int16_t *d_volt, float *d_power, int64_t n, void *cuda_stream);
+
 /* The whole chain from HOST buffers (per-beam threads copy their input to the GPU;
  * north_star item 4: beam groups on separate CUDA streams with overlapped host-to-device copies).
  * h_in [nbeams][nchans][nsamps] (pinned memory overlaps best); the clipped data is NOT copied back.

@@ -190,3 +190,12 @@ def power_i16(volt: np.ndarray) -> np.ndarray:
     out = np.empty(volt.shape[:-1], dtype=np.float32)
     _L().orc_power_i16(_p(volt), c_int64(out.size), _p(out))
     return out
+
+
+def mulaw_u8(x: np.ndarray, mu: float):
+    """8-bit mu-law codes of a non-negative float32 series (Eq. 5; reading G-i). Returns (codes, xmax)."""
+    assert x.dtype == np.float32 and x.flags.c_contiguous and mu > 0
+    code = np.empty(x.shape, dtype=np.uint8)
+    xmax = np.zeros(1, dtype=np.float32)
+    _L().orc_mulaw_u8(_p(x), c_int64(x.size), c_double(mu), _p(code), _p(xmax))
+    return code, float(xmax[0])

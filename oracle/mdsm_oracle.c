@@ -453,3 +453,26 @@ void orc_power_i16(const int16_t *volt, int64_t n, float *power)
         power[i] = (float)(double)(re * re + im * im);      /* int64 -> double exact, double -> float round to nearest */
     }
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * mu-law quantiser of a channelised power series, 32-bit float -> 8 bits (Eq. 5) -- SURVEY 8(f)
+ * NEXT-4.   y = Xmax * log(1 + mu |x| / Xmax) / log(1 + mu) * sign(x),  Xmax = the maximum of the series.
+ * Readings (G-i): the paper does not say how y becomes 8 bits; power is non-negative, so the
+ * code is unsigned, code = floor(255 * y / Xmax + 0.5); negative or NaN input and an all-zero series give code 0.
+ * fp64 with log1p.  Pinned by closed-form values (x = 0, x = Xmax, the mu -> 0 linear limit, monotonicity, the
+ * textbook mid-point x/Xmax = (sqrt(1+mu) - 1)/mu -> y/Xmax = 1/2).  xmax_out (may be NULL) receives Xmax.
+ * ------------------------------------------------------------------------------------------------ */
+void orc_mulaw_u8(const float *x, int64_t n, double mu, uint8_t *code, float *xmax_out)
+{
+    float xmax = 0.0f;
+    for (int64_t i = 0; i < n; ++i)
+        if (x[i] > xmax) xmax = x[i];
+    if (xmax_out) *xmax_out = xmax;
+    const double den = log1p(mu);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double v = 0.0;
+        if (xmax > 0.0f && x[i] > 0.0f) v = 255.0 * (log1p(mu * ((double)x[i] / (double)xmax)) / den);
+        code[i] = (uint8_t)floor(v + 0.5);
+    }
+}

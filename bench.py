@@ -290,6 +290,21 @@ def main():
         post["power_ms"] = statistics.mean(tp[1:])
         post["power_hbm_frac"] = 8.0 * nel / (post["power_ms"] * 1e-3) / hp
         del volt
+        # mu-law quantiser (Eq. 5, NEXT-4) on the fp32 input buffer (power is non-negative: use |x|)
+        src = work.abs_()
+        codes = torch.empty((nel,), dtype=torch.uint8, device="cuda")
+        xmax = torch.zeros(1, dtype=torch.float32, device="cuda")
+        tq = []
+        for _ in range(5):
+            out.zero_()
+            pe[0].record(stream)
+            m.mdsm_mulaw_u8(src, codes, nel, 255.0, xmax, stream)
+            pe[1].record(stream)
+            torch.cuda.synchronize()
+            tq.append(pe[0].elapsed_time(pe[1]))
+        post["mulaw_ms"] = statistics.mean(tq[1:])
+        post["mulaw_hbm_frac"] = 9.0 * nel / (post["mulaw_ms"] * 1e-3) / hp
+        del codes
 
     # ---- end to end through the host-buffer C-ABI call (H2D of the input and D2H of the events inside) ----
     e2e = None

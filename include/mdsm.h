@@ -124,6 +124,13 @@ int mdsm_detrend(mdsm_plan *plan, float *d_series, int beam0, int nb, double *d_
  * null / misaligned buffers or n < 0. */
 int mdsm_power_i16(const int16_t *d_volt, float *d_power, int64_t n, void *cuda_stream);
 
+/* mu-law quantiser of a (non-negative) float power series to 8 bits (Eq. 5):
+ *   Xmax = max x;  code = floor(255 * log(1 + mu x / Xmax) / log(1 + mu) + 0.5)   (fp64; x <= 0, NaN or Xmax == 0 -> 0).
+ * d_x [n] floats, d_code [n] bytes, both 16-byte aligned device buffers; d_xmax: one device float that receives Xmax
+ * (the decoder needs it).  Asynchronous on cuda_stream; needs no plan.  MDSM_EINVAL for null / misaligned buffers,
+ * n < 0 or mu <= 0. */
+int mdsm_mulaw_u8(const float *d_x, uint8_t *d_code, int64_t n, double mu, float *d_xmax, void *cuda_stream);
+
 /* The whole chain from HOST buffers (per-beam threads copy their input to the GPU;
  * north_star item 4: beam groups on separate CUDA streams with overlapped host-to-device copies).
  * h_in [nbeams][nchans][nsamps] (pinned memory overlaps best); the clipped data is NOT copied back.

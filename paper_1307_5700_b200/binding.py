@@ -17,7 +17,7 @@ __all__ = [
     "EVENT_DTYPE", "MdsmError", "lib_path",
     "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
-    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_pipeline_host", "mdsm_measure_add_peak",
+    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
 ]
 
 MDSM_F32, MDSM_U8 = 0, 1
@@ -73,6 +73,8 @@ def _load():
     L.mdsm_detrend.argtypes = [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p]
     L.mdsm_power_i16.restype = c_int
     L.mdsm_power_i16.argtypes = [c_void_p, c_void_p, c_int64, c_void_p]
+    L.mdsm_mulaw_u8.restype = c_int
+    L.mdsm_mulaw_u8.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]
     L.mdsm_pipeline_host.restype = c_int
     L.mdsm_pipeline_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, c_double, c_void_p,
                                      c_int64, POINTER(c_uint64), c_int]
@@ -185,6 +187,10 @@ def mdsm_detrend(plan, d_series, beam0, nb, d_params=None, stream=None) -> None:
 
 def mdsm_power_i16(d_volt, d_power, n, stream=None) -> None:
     _check(_L.mdsm_power_i16(_ptr(d_volt), _ptr(d_power), n, _stream(stream)))
+
+
+def mdsm_mulaw_u8(d_x, d_code, n, mu, d_xmax, stream=None) -> None:
+    _check(_L.mdsm_mulaw_u8(_ptr(d_x), _ptr(d_code), n, mu, _ptr(d_xmax), _stream(stream)))
 
 
 def mdsm_pipeline_host(plan, h_in, window, k_chan, k_spec, snr_thresh, h_events, max_events, nstreams=4,

@@ -458,11 +458,8 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
     if (stages > 12) stages = 12;
     MDSM_REQUIRE(stages >= 2, "tiled kernel: staged rows too large for shared memory");
     const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t) + 16;
-    static thread_local size_t smem_set = 0;
-    if (smem > smem_set) {
-        MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        smem_set = smem;
-    }
+    // per launch: the attribute belongs to the current device's copy of the kernel, and the call costs microseconds
+    MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     TiledArgs a;
     a.in = d_in; a.out = d_out;
     a.row_start = tt.d_row_start; a.warp_tab = (const unsigned long long *)tt.d_warp_tab; a.sigma = tt.d_sigma;

@@ -1,0 +1,56 @@
+"""Seeded random plans (channel count, band, sampling time, DM grid, beams, buffer length) through both dedispersion
+kernels against the oracle: the tile tables, shears, parts, ragged DM blocks and edge tiles of whatever geometry the
+plan picks.  u8 bit-exact, fp32 inside the north_star tolerance."""
+import numpy as np
+import pytest
+
+import oracle
+
+from gpu_util import Plan, out_to_numpy
+
+pytestmark = pytest.mark.gpu
+
+
+def _shape(seed):
+    g = np.random.default_rng(1000 + seed)
+    nchans = int(g.choice([5, 24, 100, 257, 300, 512, 700]))
+    bw = float(g.choice([5.0, 20.0, 32.0]))
+    f_top = float(g.choice([418.0, 1400.0, 150.0]))
+    if f_top - bw < 40.0:
+        bw = 5.0
+    tsamp = float(g.choice([51.2e-6, 64e-6, 1e-4]))
+    ndms = int(g.integers(1, 130))
+    dm_low = float(g.choice([0.0, 3.7, 20.0]))
+    dm_step = float(g.choice([0.05, 0.1, 0.13, 0.25]))
+    nbeams = int(g.integers(1, 4))
+    args = [nbeams, nchans, f_top, -bw / nchans, tsamp, 0, dm_low, dm_step, ndms]
+    d = oracle.delay_table(nchans, f_top, -bw / nchans, tsamp, dm_low, dm_step, ndms)
+    nsamps = int(d.max()) + int(g.integers(1500, 6000))
+    nsamps += (-nsamps) % int(g.choice([1, 4, 8, 16]))
+    args[5] = nsamps
+    return tuple(args), d
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("MDSM_FUZZ_SEEDS", "24"))))
+def test_random_plan(seed):
+    import torch
+    args, d = _shape(seed)
+    if (args[5] - int(d.max())) * args[0] * args[8] * args[1] > 3e9:
+        pytest.skip("oracle too slow for this draw")
+    g = np.random.default_rng(seed)
+    nb, nc, ns = args[0], args[1], args[5]
+    xf = (g.normal(size=(nb, nc, ns)) * g.uniform(0.5, 2.0, size=(1, nc, 1)) + 3.0).astype(np.float32)
+    xu = np.clip(np.rint(g.normal(size=(nb, nc, ns)) * 50 + 100), 0, 255).astype(np.uint8)
+    with Plan(args) as p:
+        n = p.nsamps_out
+        assert np.array_equal(p.delays(), d)
+        for x in (xf, xu):
+            ref, ab = oracle.dedisperse(x, d)
+            for kernel in (0, 1):
+                out = p.dedisperse(torch.from_numpy(x).cuda(), kernel=kernel)
+                got = out_to_numpy(out, n)
+                if x.dtype == np.uint8:
+                    assert np.array_equal(got, ref), (args, kernel)
+                else:
+                    assert np.all(np.abs(got.astype(np.float64) - ref) <= 1e-5 * ab + 1e-6), (args, kernel)
+                assert bool((out[:, :, n:] == -7).all())

@@ -54,3 +54,37 @@ def test_random_plan(seed):
                 else:
                     assert np.all(np.abs(got.astype(np.float64) - ref) <= 1e-5 * ab + 1e-6), (args, kernel)
                 assert bool((out[:, :, n:] == -7).all())
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_plan_u8_chain_bit_exact(seed):
+    """clip -> dedisperse -> detect from host buffers (mdsm_pipeline_host) on random plans: the event list must equal
+    the oracle's, bit for bit, for uint8 input."""
+    import paper_1307_5700_b200 as m
+    args, d = _shape(100 + seed)
+    args = list(args)
+    W = int(np.random.default_rng(seed).choice([8, 16, 64]))
+    args[5] += (-args[5]) % W                                   # the clip wants nsamps % window == 0
+    if (args[5] - int(d.max())) * args[0] * args[8] * args[1] > 3e9:
+        pytest.skip("oracle too slow for this draw")
+    g = np.random.default_rng(50 + seed)
+    nb, nc, ns = args[0], args[1], args[5]
+    x = np.clip(np.rint(g.normal(size=(nb, nc, ns)) * 10 + 64), 0, 255).astype(np.uint8)
+    for _ in range(4):                                          # narrow-band bursts, broadband spikes, one pulse
+        b, c, t = int(g.integers(nb)), int(g.integers(nc)), int(g.integers(ns - 200))
+        x[b, c, t:t + 150] = np.minimum(x[b, c, t:t + 150].astype(int) + 60, 255)
+        x[b, :, int(g.integers(ns))] = 200
+    k = int(g.integers(args[8]))
+    t0 = int(g.integers(0, ns - int(d.max()) - 1))
+    x[0, np.arange(nc), t0 + d[k]] = np.minimum(x[0, np.arange(nc), t0 + d[k]].astype(int) + 90, 255)
+    xo = x.copy()
+    oracle.rfi_clip(xo, W, 5.0, 5.0)
+    ref, _ = oracle.dedisperse(xo, d)
+    ev_o, cnt_o, _ = oracle.detect(ref, ref.shape[2], 5.0)
+    with Plan(tuple(args)) as p:
+        hev = np.zeros(1 << 18, dtype=m.EVENT_DTYPE)
+        rc, cnt = m.mdsm_pipeline_host(p.h, x, W, 5.0, 5.0, 5.0, hev, len(hev), 3)
+        assert rc == m.MDSM_OK and cnt == cnt_o, (args, cnt, cnt_o)
+        hev = hev[:cnt]
+        hev = hev[np.lexsort((hev["t"], hev["dm_idx"], hev["beam"]))]
+        assert np.array_equal(hev, ev_o), args

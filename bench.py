@@ -169,6 +169,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--nstreams", type=int, default=8)
+    ap.add_argument("--pairs", type=int, default=-1, help="plan option pair_presum (fp32: exact channel-pair pre-sums); -1 = plan default")
     ap.add_argument("--postprocess", type=int, default=0,
                     help="median window W: also time mdsm_median_filter(W) + mdsm_detrend on the dedispersed series (fp32 "
                          "configs; reported beside the chain, not part of `value`)")
@@ -203,6 +204,8 @@ def main():
     work = torch.empty_like(pristine)
     plan = m.mdsm_plan_create(*cfg.plan_args())
     m.mdsm_plan_set_option(plan, "dedisp_kernel", args.kernel)
+    if args.pairs >= 0:
+        m.mdsm_plan_set_option(plan, "pair_presum", args.pairs)
     if args.geom >= 0:
         m.mdsm_plan_set_option(plan, "tiled_geom_" + cfg.dtype, args.geom)
     nso = m.mdsm_plan_nsamps_out(plan)

@@ -142,6 +142,9 @@ struct TiledArgs {
     const int32_t *row_start;             // [nblk][nslab*CS]  first staged sample of the row, relative to tile_t0
     const unsigned long long *warp_tab;   // [nblk][nslab][NW][CS] window entries (format: gen_chain.py)
     const int32_t *sigma;                 // [DB] output time shear per DM of a block
+    const int32_t *src_row;               // pair mode: [nblk][nslab*CS] source row of staged row r (-1: none); else nullptr
+    const int32_t *nslab_blk;             // pair mode: [nblk] slabs of the block; else nullptr
+    int nrows_src;                        // rows per beam of the staged source (nchans, or the pre-summed copy's row count)
     int beam0, nchans, nslab, slabs_per_part, ndms;
     long long nsamps, nsamps_out;
     int row_elems, stages;
@@ -154,6 +157,10 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
     using In = float; using Out = float; using Acc = unsigned long long;
     using Slab = SlabF32<D_, T_, NOFF_>;
     static_assert(T_ % 4 == 0 && (T_ / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
+};
+// pair pre-sum mode: same data types as TraitsF32, loop with skip bits and per-slot dispatchers (gen_chain.py: gen_f32p)
+template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32P : TraitsF32<D_, T_, NW_, CS_, NOFF_> {
+    using Slab = SlabF32P<D_, T_, NOFF_>;
 };
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
@@ -215,17 +222,20 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
             int blk, tt, bb;
             a.walk.decode(tile, blk, tt, bb);
             const long long tile_t0 = (long long)tt * (32 * T);
-            const In *beam_in = reinterpret_cast<const In *>(a.in) + (size_t)(a.beam0 + bb) * a.nchans * (size_t)a.nsamps;
+            const In *beam_in = reinterpret_cast<const In *>(a.in) + (size_t)(a.beam0 + bb) * a.nrows_src * (size_t)a.nsamps;
             const int32_t *rs = a.row_start + (size_t)blk * ncp;
+            const int32_t *sr = a.src_row ? a.src_row + (size_t)blk * ncp : nullptr;
             const unsigned long long *wt = a.warp_tab + (size_t)blk * a.nslab * NW * CS;
-            for (int slab = 0; slab < a.nslab; ++slab) {
+            const int nslab_b = a.nslab_blk ? a.nslab_blk[blk] : a.nslab;
+            for (int slab = 0; slab < nslab_b; ++slab) {
                 if (!first_lap) mbar_wait_sleep(&empty[st], ph);
                 if (lane < CS) {
-                    const int c = slab * CS + lane;
+                    const int r = slab * CS + lane;
+                    const int c = sr ? sr[r] : (r < a.nchans ? r : -1);      // source row of staged row r
                     uint32_t bytes = 0;
                     long long lo = 0, g0 = 0;
-                    if (c < a.nchans) {
-                        g0 = tile_t0 + rs[c];
+                    if (c >= 0) {
+                        g0 = tile_t0 + rs[r];
                         lo = g0 < 0 ? 0 : g0;
                         long long hi = g0 + a.row_elems;
                         if (hi > a.nsamps) hi = a.nsamps;
@@ -258,12 +268,14 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
         const long long tile_t0 = (long long)tt * (32 * T);
         const int b = a.beam0 + bb;
 #pragma unroll 1
-        for (int s0 = 0; s0 < a.nslab; s0 += a.slabs_per_part) {
+        const int nslab_b = a.nslab_blk ? a.nslab_blk[blk] : a.nslab;
+#pragma unroll 1
+        for (int s0 = 0; s0 < nslab_b; s0 += a.slabs_per_part) {
 #pragma unroll
             for (int j = 0; j < D; ++j)
 #pragma unroll
                 for (int i = 0; i < AW; ++i) acc[j][i] = 0;      // (+0.f, +0.f) / (0, 0)
-            const int s1 = min(a.nslab, s0 + a.slabs_per_part);
+            const int s1 = min(nslab_b, s0 + a.slabs_per_part);
 #pragma unroll 1
             for (int slab = s0; slab < s1; ++slab) {
                 mbar_wait(&full[st], ph);
@@ -311,6 +323,33 @@ __global__ void __launch_bounds__(256) widen_u8_kernel(const uint2 *__restrict__
         a.x = __byte_perm(v.x, 0, 0x4140); a.y = __byte_perm(v.x, 0, 0x4342);
         a.z = __byte_perm(v.y, 0, 0x4140); a.w = __byte_perm(v.y, 0, 0x4342);
         out[i] = a;
+    }
+}
+
+// Pair pre-sum (fp32): y[row][t] = x[c][t] + x[c+1][t + delta], row = (channel pair (c, c+1), delay difference delta).
+// delay(d, c+1) - delay(d, c) takes few values over the DM grid, so out[d][t] = sum over pairs of
+// y[(pair, delta(d, pair))][t + delay(d, c)]: the same terms, added two at a time.
+__global__ void __launch_bounds__(256) pair_presum_kernel(const float *__restrict__ in, float *__restrict__ y,
+                                                          const int32_t *__restrict__ yrow_chan, const int32_t *__restrict__ yrow_delta,
+                                                          int beam0, int nchans, int nyrows, long long nsamps)
+{
+    const int row = blockIdx.y, b = beam0 + blockIdx.z;
+    const int c = yrow_chan[row], delta = yrow_delta[row];
+    const float *x0 = in + ((size_t)b * nchans + c) * (size_t)nsamps;
+    const float *x1 = x0 + nsamps;
+    float *o = y + ((size_t)b * nyrows + row) * (size_t)nsamps;
+    const long long t0 = ((long long)blockIdx.x * 256 + threadIdx.x) * 4;
+    if (t0 >= nsamps) return;
+    if (t0 + 3 < nsamps) {
+        const float4 a = *reinterpret_cast<const float4 *>(x0 + t0);
+        float4 r;
+        r.x = a.x + (t0 + delta < nsamps ? x1[t0 + delta] : 0.0f);
+        r.y = a.y + (t0 + 1 + delta < nsamps ? x1[t0 + 1 + delta] : 0.0f);
+        r.z = a.z + (t0 + 2 + delta < nsamps ? x1[t0 + 2 + delta] : 0.0f);
+        r.w = a.w + (t0 + 3 + delta < nsamps ? x1[t0 + 3 + delta] : 0.0f);
+        *reinterpret_cast<float4 *>(o + t0) = r;
+    } else {
+        for (long long t = t0; t < nsamps; ++t) o[t] = x0[t] + (t + delta < nsamps ? x1[t + delta] : 0.0f);
     }
 }
 
@@ -432,6 +471,116 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, bool two
     return true;
 }
 
+// Pair mode tables: the rows a DM block stages are (channel pair, delay difference) rows of the pre-summed copy; a row
+// is used by the DMs of the block whose delay difference for that pair equals the row's, the others carry offset 15
+// (= skip) in the window entry.  Same geometry, shear and entry format as build_tables.
+static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTables &tt, std::vector<int32_t> &h_rs,
+                               std::vector<unsigned long long> &h_tab, std::vector<int32_t> &h_sigma, std::vector<int32_t> &h_src,
+                               std::vector<int32_t> &h_nslab, std::vector<int32_t> &h_ychan, std::vector<int32_t> &h_ydelta)
+{
+    if (p->nchans % 2 || p->nchans < 2 || g.NOFF > 15) return false;
+    const int al = 4, DB = g.D * g.NW, TT = 32 * g.T, np = p->nchans / 2;
+    const int nblk = (p->ndms + DB - 1) / DB;
+    auto dly = [&](int d, int c) { return (long long)p->h_delay[(size_t)std::min(d, p->ndms - 1) * p->nchans + c]; };
+    // rows of the pre-summed copy: every delay difference a pair takes over the whole DM grid
+    std::vector<int> ybase(np), ylo(np);
+    h_ychan.clear(); h_ydelta.clear();
+    for (int q = 0; q < np; ++q) {
+        long long lo = 1LL << 60, hi = -1;
+        for (int d = 0; d < p->ndms; ++d) {
+            const long long dl = dly(d, 2 * q + 1) - dly(d, 2 * q);
+            lo = std::min(lo, dl); hi = std::max(hi, dl);
+        }
+        if (lo < 0 || hi - lo > 64) return false;
+        ybase[q] = (int)h_ychan.size(); ylo[q] = (int)lo;
+        for (long long dl = lo; dl <= hi; ++dl) { h_ychan.push_back(2 * q); h_ydelta.push_back((int32_t)dl); }
+    }
+    const double f_lo = p->f_top + (p->nchans - 1) * p->foff;
+    const double smax = 4.148808e3 * p->dm_step * (1.0 / (f_lo * f_lo) - 1.0 / (p->f_top * p->f_top)) / p->tsamp;
+    h_sigma.resize(DB);
+    for (int dl = 0; dl < DB; ++dl) h_sigma[dl] = (int32_t)llround(0.5 * smax * dl);
+    // per block: the list of (pair, delta) rows some DM of the block uses
+    struct Row { int q, delta; };
+    std::vector<std::vector<Row>> rows(nblk);
+    int nslab_max = 0;
+    h_nslab.resize(nblk);
+    for (int blk = 0; blk < nblk; ++blk) {
+        for (int q = 0; q < np; ++q) {
+            std::vector<int> seen;
+            for (int dl = 0; dl < DB; ++dl) {
+                const int d = blk * DB + dl;
+                const int de = (int)(dly(d, 2 * q + 1) - dly(d, 2 * q));
+                if (std::find(seen.begin(), seen.end(), de) == seen.end()) seen.push_back(de);
+            }
+            std::sort(seen.begin(), seen.end());
+            for (int de : seen) rows[blk].push_back({q, de});
+        }
+        h_nslab[blk] = ((int)rows[blk].size() + g.CS - 1) / g.CS;
+        nslab_max = std::max(nslab_max, h_nslab[blk]);
+    }
+    const int ncp = nslab_max * g.CS;
+    h_rs.assign((size_t)nblk * ncp, 0);
+    h_src.assign((size_t)nblk * ncp, -1);
+    h_tab.assign((size_t)nblk * nslab_max * g.NW * g.CS, 0ULL);
+    auto e_of = [&](int blk, int dl, int c) { return dly(blk * DB + dl, c) - h_sigma[dl]; };
+    auto uses = [&](int blk, int dl, const Row &r) { const int d = blk * DB + dl; return dly(d, 2 * r.q + 1) - dly(d, 2 * r.q) == r.delta; };
+    long long max_need = 0;
+    int worst = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int row_elems = (int)((max_need + al - 1) / al * al);
+        if (pass == 1 && (worst >= g.NOFF || (long long)g.CS * row_elems * 4 >= (1 << 18))) return false;
+        for (int blk = 0; blk < nblk; ++blk)
+            for (int ri = 0; ri < (int)rows[blk].size(); ++ri) {
+                const Row &r = rows[blk][ri];
+                const int c = 2 * r.q;
+                long long mn = 1LL << 60;
+                for (int dl = 0; dl < DB; ++dl)
+                    if (uses(blk, dl, r)) mn = std::min(mn, e_of(blk, dl, c));
+                const long long rs = floor_to(mn, al);
+                if (pass == 1) {
+                    h_rs[(size_t)blk * ncp + ri] = (int32_t)rs;
+                    h_src[(size_t)blk * ncp + ri] = ybase[r.q] + (r.delta - ylo[r.q]);
+                }
+                const int slab = ri / g.CS, rr = ri % g.CS;
+                const bool last = (rr == g.CS - 1) || (ri == (int)rows[blk].size() - 1);
+                for (int w = 0; w < g.NW; ++w) {
+                    long long wmn = 1LL << 60, wmx = -(1LL << 60), e[8];
+                    bool use[8];
+                    for (int j = 0; j < g.D; ++j) {
+                        use[j] = uses(blk, w * g.D + j, r);
+                        e[j] = e_of(blk, w * g.D + j, c) - rs;
+                        if (use[j]) { wmn = std::min(wmn, e[j]); wmx = std::max(wmx, e[j]); }
+                    }
+                    const bool any = wmx >= wmn;
+                    const long long A = any ? floor_to(wmn, al) : 0;
+                    const int chunks = any ? (g.T + (int)(wmx - A) + al - 1) / al : g.T / al;
+                    if (pass == 0) {
+                        if (any) {
+                            worst = std::max(worst, (int)(wmx - A));
+                            max_need = std::max(max_need, A + 31LL * g.T + (long long)al * chunks);
+                        }
+                        continue;
+                    }
+                    unsigned long long lo = (unsigned long long)(((long long)rr * row_elems + A) * 4);
+                    for (int i = 0; i < chunks - g.T / al; ++i) lo |= 1ULL << (28 + i);
+                    if (last) lo |= 1ULL << 31;
+                    unsigned long long hi = 0;
+                    for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(use[j] ? (e[j] - A) : 0x80) << (8 * j);   // bit 7: skips the row
+                    h_tab[(((size_t)blk * nslab_max + slab) * g.NW + w) * g.CS + rr] = lo | (hi << 32);
+                }
+            }
+        if (pass == 1) {
+            tt.row_words = row_elems;
+        }
+    }
+    tt.dms_per_warp = g.D; tt.warps = g.NW; tt.tpt = g.T; tt.cs = g.CS;
+    tt.dm_block = DB; tt.n_dm_blocks = nblk; tt.tile_t = TT;
+    tt.max_off = worst;
+    tt.sigma_max = *std::max_element(h_sigma.begin(), h_sigma.end());
+    tt.pairs = true; tt.nslab_max = nslab_max; tt.nyrows = (int)h_ychan.size();
+    return true;
+}
+
 template <typename V> static bool upload(V **dptr, const std::vector<V> &h)
 {
     if (cudaMalloc((void **)dptr, h.size() * sizeof(V)) != cudaSuccess) return false;
@@ -443,7 +592,10 @@ static void free_tables(TiledTables *tt)
     cudaFree(tt->d_row_start);
     cudaFree(tt->d_warp_tab);
     cudaFree(tt->d_sigma);
+    cudaFree(tt->d_src_row); cudaFree(tt->d_nslab_blk); cudaFree(tt->d_yrow_chan); cudaFree(tt->d_yrow_delta);
     tt->d_row_start = nullptr; tt->d_warp_tab = nullptr; tt->d_sigma = nullptr;
+    tt->d_src_row = nullptr; tt->d_nslab_blk = nullptr; tt->d_yrow_chan = nullptr; tt->d_yrow_delta = nullptr;
+    tt->pairs = false;
     tt->ok = false;
 }
 
@@ -463,8 +615,11 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
     TiledArgs a;
     a.in = d_in; a.out = d_out;
     a.row_start = tt.d_row_start; a.warp_tab = (const unsigned long long *)tt.d_warp_tab; a.sigma = tt.d_sigma;
-    a.beam0 = beam0; a.nchans = p->nchans; a.nslab = nslab; a.ndms = p->ndms;
-    a.slabs_per_part = part_chans > 0 ? part_chans / Tr::CS : nslab;
+    a.src_row = tt.pairs ? tt.d_src_row : nullptr;
+    a.nslab_blk = tt.pairs ? tt.d_nslab_blk : nullptr;
+    a.nrows_src = tt.pairs ? tt.nyrows : p->nchans;
+    a.beam0 = beam0; a.nchans = p->nchans; a.nslab = tt.pairs ? tt.nslab_max : nslab; a.ndms = p->ndms;
+    a.slabs_per_part = part_chans > 0 ? part_chans / Tr::CS : (tt.pairs ? tt.nslab_max : nslab);
     a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out;
     a.row_elems = tt.row_words; a.stages = stages;
     a.walk.nblk = tt.n_dm_blocks;
@@ -478,6 +633,7 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
 }
 
 template <int G> using GeomF32 = TraitsF32<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
+template <int G> using GeomF32P = TraitsF32P<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
 template <int G> using GeomU16 = TraitsU16<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
 template <int G> using GeomU16P = TraitsU16P<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
 
@@ -505,6 +661,20 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
     free_tables(&p->tiled_u8);
     // Rows must be 16-byte aligned for the bulk copies.  tiled_geom_* < 0 = automatic: the first compiled geometry
     // whose register window takes this plan's delay spread (coarser DM grids need fewer DMs per warp).
+    if (p->pair_presum && p->nsamps % 4 == 0) {
+        std::vector<int32_t> rs, sig, src, nsl, yc, yd;
+        std::vector<unsigned long long> tab;
+        TiledTables &tt = p->tiled_f32;
+        if (build_tables_pairs(p, kGeomF32[0], tt, rs, tab, sig, src, nsl, yc, yd)) {
+            if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig) ||
+                !upload(&tt.d_src_row, src) || !upload(&tt.d_nslab_blk, nsl) || !upload(&tt.d_yrow_chan, yc) || !upload(&tt.d_yrow_delta, yd)) {
+                mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+                return MDSM_ECUDA;
+            }
+            tt.geom = 0;
+            tt.ok = true;
+        }
+    }
     if (p->nsamps % 4 == 0 && p->tiled_geom_f32 < kNumGeomF32)
         for (int g = 0; g < kNumGeomF32 && !p->tiled_f32.ok; ++g) {
             if (p->tiled_geom_f32 >= 0 && g != p->tiled_geom_f32) continue;
@@ -528,6 +698,9 @@ void mdsm_tiled_free_tables(mdsm_plan *p)
     cudaFree(p->d_widen);
     p->d_widen = nullptr;
     p->widen_bytes = 0;
+    cudaFree(p->d_pairs);
+    p->d_pairs = nullptr;
+    p->pairs_bytes = 0;
 }
 
 int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
@@ -535,6 +708,24 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
 {
     if (dtype == MDSM_F32) {
         const TiledTables &tt = p->tiled_f32;
+        if (tt.pairs) {
+            // pre-sum the channel pairs of these beams into the plan's scratch (allocated on first use), then walk its rows
+            const size_t need = (size_t)p->nbeams * tt.nyrows * (size_t)p->nsamps * sizeof(float);
+            if (p->pairs_bytes < need) {
+                cudaFree(p->d_pairs);
+                p->d_pairs = nullptr;
+                p->pairs_bytes = 0;
+                MDSM_CUDA_TRY(cudaMalloc(&p->d_pairs, need));
+                p->pairs_bytes = need;
+            }
+            dim3 grid((unsigned)((p->nsamps / 4 + 255) / 256), tt.nyrows, nb);
+            MDSM_REQUIRE(tt.nyrows <= 65535 && nb <= 65535, "pair pre-sum: grid too large");
+            pair_presum_kernel<<<grid, 256, 0, st>>>((const float *)d_in, (float *)p->d_pairs, tt.d_yrow_chan, tt.d_yrow_delta, beam0,
+                                                     p->nchans, tt.nyrows, p->nsamps);
+            MDSM_CUDA_TRY(cudaGetLastError());
+            p->launches += 1;
+            return launch_tiled<GeomF32P<0>>(p, tt, p->d_pairs, beam0, nb, d_out, 0, st);
+        }
         switch (tt.geom) {
             case 0: return launch_tiled<GeomF32<0>>(p, tt, d_in, beam0, nb, d_out, 0, st);
             case 1: return launch_tiled<GeomF32<1>>(p, tt, d_in, beam0, nb, d_out, 0, st);

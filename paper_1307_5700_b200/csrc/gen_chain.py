@@ -45,15 +45,22 @@ def tree_bits(e, j):
         e(f"and.b32 tm, hi, {1 << (8 * j + bit)}; setp.ne.u32 b{bit}, tm, 0;")
 
 
+SKIP_LEAF = False        # set while generating a loop whose table entries may carry offset 15 = "this DM skips the row"
+
+
 def tree_branch(e, j, noff):
     """branch to B{j}_{o}: at most 4 conditional direct branches, ~2 taken"""
     def leaf(k):
+        if SKIP_LEAF and k == 15:
+            return f"B{j}_15"
         return f"B{j}_{k}" if k < noff else f"B{j}_0"
     e(f"@b3 bra.uni X{j}_8; @b2 bra.uni X{j}_4; @b1 bra.uni X{j}_2; @b0 bra.uni {leaf(1)}; bra.uni {leaf(0)};")
 
 
 def tree_stubs(e, j, noff):
     def leaf(k):
+        if SKIP_LEAF and k == 15:
+            return f"B{j}_15"
         return f"B{j}_{k}" if k < noff else f"B{j}_0"
     e(f"X{j}_2: @b0 bra.uni {leaf(3)}; bra.uni {leaf(2)};")
     e(f"X{j}_4: @b1 bra.uni X{j}_6; @b0 bra.uni {leaf(5)}; bra.uni {leaf(4)};")
@@ -78,6 +85,15 @@ class Emit:
 
 
 def gen_f32(D, T, NOFF):
+    global SKIP_LEAF
+    SKIP_LEAF = False
+    try:
+        return _gen_f32(D, T, NOFF)
+    finally:
+        SKIP_LEAF = False
+
+
+def _gen_f32(D, T, NOFF):
     assert T % 4 == 0 and D <= 4
     A2 = T // 2
     NCH = nchunks(T, NOFF, 4)
@@ -117,7 +133,7 @@ def gen_f32(D, T, NOFF):
     head()
     for j in range(D):
         last = j == D - 1
-        for k in range(NOFF):
+        for k in list(range(NOFF)) + ([15] if SKIP_LEAF else []):
             m = k // 2
             e(f"B{j}_{k}:")
             if last:
@@ -127,7 +143,7 @@ def gen_f32(D, T, NOFF):
             else:
                 tree_bits(e, j + 1)
             body = ""
-            for i in range(A2):
+            for i in range(A2 if k < NOFF else 0):
                 a = j * A2 + i
                 if k % 2 == 0:
                     body += f"add.rn.f32x2 %{a}, %{a}, w{m + i}; "
@@ -158,6 +174,81 @@ def gen_f32(D, T, NOFF):
     s.append('        : "r"(sbase), "r"(tab) : "memory");')
     s.append("}\n")
     s.append(f"template <> struct SlabF32<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned long long (&a)[{D}][{A2}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
+    return "\n".join(s)
+
+
+def gen_f32p(D, T, NOFF):
+    """fp32 loop of the pair pre-sum mode: a staged row is used by a SUBSET of the warp's DMs (bit 7 of a DM's offset
+    byte = "skips this row").  The chain hops from one participating DM to the next: after its adds a block tests the
+    skip bits of the DMs behind it (one predicated branch each) and enters the shared dispatcher DISP_j' of the first
+    participant, or the loop tail when none is left.  One loop head (not copied), one dispatcher per DM slot."""
+    assert T % 4 == 0 and D <= 4
+    A2 = T // 2
+    NCH = nchunks(T, NOFF, 4)
+    W2 = NCH * 2
+    base_ch = T // 4
+    assert NCH - base_ch <= 3
+    nacc = D * A2
+    SB, TAB = nacc, nacc + 1
+    name = f"slab_f32p_{D}_{T}_{NOFF}"
+    e = Emit()
+    e("{")
+    e(f".reg .b64 w<{W2}>;")
+    e(".reg .b32 lo, hi, p, tp, tm;")
+    e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3, s0, s1, s2, s3;")
+    e(".reg .f32 a0, a1, x0, x1, y0, y1;")
+
+    def skip_preds(first):
+        for j in range(first, D):
+            e(f"and.b32 tm, hi, {0x80 << (8 * j)}; setp.ne.u32 s{j}, tm, 0;")
+
+    def hop(first):
+        e(" ".join(f"@!s{j} bra.uni DISP{j};" for j in range(first, D)) + " bra.uni TAIL;")
+
+    e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    e("bra.uni HEAD;")
+    e("TAIL:")
+    e("@pl bra.uni Bend;")
+    e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
+    e("HEAD:")
+    e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
+    for i in range(NCH - base_ch):
+        e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
+    e("setp.lt.s32 pl, lo, 0;")
+    skip_preds(0)
+    for i in range(NCH):
+        pred = f"@q{i - base_ch} " if i >= base_ch else ""
+        e(f"{pred}ld.shared.v2.b64 {{w{2 * i}, w{2 * i + 1}}}, [p+{16 * i}];")
+    hop(0)
+    for j in range(D):
+        e(f"DISP{j}:")
+        tree_bits(e, j)
+        tree_branch(e, j, NOFF)
+        tree_stubs(e, j, NOFF)
+        for k in range(NOFF):
+            m = k // 2
+            e(f"B{j}_{k}:")
+            skip_preds(j + 1)
+            body = ""
+            for i in range(A2):
+                a = j * A2 + i
+                if k % 2 == 0:
+                    body += f"add.rn.f32x2 %{a}, %{a}, w{m + i}; "
+                else:
+                    body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, w{m + i}; mov.b64 {{y0,y1}}, w{m + i + 1}; "
+                             f"add.f32 a0, a0, x1; add.f32 a1, a1, y0; mov.b64 %{a}, {{a0,a1}}; ")
+            e(body)
+            hop(j + 1)
+    e("Bend:")
+    e("}")
+    s = [f"// f32x2 slab loop, pair pre-sum mode: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
+    s.append(f"__device__ __forceinline__ void {name}(unsigned long long (&acc)[{D}][{A2}], unsigned sbase, unsigned tab)\n{{")
+    s.append("    asm volatile(")
+    s += e.lines
+    s.append("        : " + ", ".join(f'"+l"(acc[{j}][{i}])' for j in range(D) for i in range(A2)))
+    s.append('        : "r"(sbase), "r"(tab) : "memory");')
+    s.append("}\n")
+    s.append(f"template <> struct SlabF32P<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned long long (&a)[{D}][{A2}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
     return "\n".join(s)
 
 
@@ -335,6 +426,7 @@ def gen_u16p(D, T, NOFF):
 F32_VARIANTS = [(4, 28, 12), (4, 20, 12), (2, 28, 12)]
 U16_VARIANTS = [(4, 40, 16)]
 U16P_VARIANTS = [(2, 40, 12), (3, 40, 14)]
+F32P_VARIANTS = [(4, 28, 12)]
 
 
 def main(out):
@@ -342,12 +434,15 @@ def main(out):
     parts.append("template <int D, int T, int NOFF> struct SlabF32;   // packed f32x2 slab loop\n")
     parts.append("template <int D, int T, int NOFF> struct SlabU16;   // packed u16x2 slab loop\n")
     parts.append("template <int D, int T, int NOFF> struct SlabU16P;  // two-phase packed u16x2 slab loop\n")
+    parts.append("template <int D, int T, int NOFF> struct SlabF32P;  // packed f32x2 slab loop of the pair pre-sum mode\n")
     for v in F32_VARIANTS:
         parts.append(gen_f32(*v))
     for v in U16_VARIANTS:
         parts.append(gen_u16(*v))
     for v in U16P_VARIANTS:
         parts.append(gen_u16p(*v))
+    for v in F32P_VARIANTS:
+        parts.append(gen_f32p(*v))
     txt = "\n".join(parts)
     if os.path.exists(out) and open(out).read() == txt:
         return

@@ -328,28 +328,37 @@ __global__ void __launch_bounds__(256) widen_u8_kernel(const uint2 *__restrict__
 
 // Pair pre-sum (fp32): y[row][t] = x[c][t] + x[c+1][t + delta], row = (channel pair (c, c+1), delay difference delta).
 // delay(d, c+1) - delay(d, c) takes few values over the DM grid, so out[d][t] = sum over pairs of
-// y[(pair, delta(d, pair))][t + delay(d, c)]: the same terms, added two at a time.
+// y[(pair, delta(d, pair))][t + delay(d, c)]: the same terms, added two at a time.  One CTA column per pair writes all
+// the rows of that pair (consecutive in y), so x is read once.
 __global__ void __launch_bounds__(256) pair_presum_kernel(const float *__restrict__ in, float *__restrict__ y,
-                                                          const int32_t *__restrict__ yrow_chan, const int32_t *__restrict__ yrow_delta,
+                                                          const int32_t *__restrict__ pair_row0, const int32_t *__restrict__ yrow_delta,
                                                           int beam0, int nchans, int nyrows, long long nsamps)
 {
-    const int row = blockIdx.y, b = beam0 + blockIdx.z;
-    const int c = yrow_chan[row], delta = yrow_delta[row];
-    const float *x0 = in + ((size_t)b * nchans + c) * (size_t)nsamps;
+    const int q = blockIdx.y, b = beam0 + blockIdx.z;
+    const int row0 = pair_row0[q], nv = pair_row0[q + 1] - row0;
+    const int dlo = yrow_delta[row0];
+    const float *x0 = in + ((size_t)b * nchans + 2 * q) * (size_t)nsamps;
     const float *x1 = x0 + nsamps;
-    float *o = y + ((size_t)b * nyrows + row) * (size_t)nsamps;
+    float *o = y + ((size_t)b * nyrows + row0) * (size_t)nsamps;
     const long long t0 = ((long long)blockIdx.x * 256 + threadIdx.x) * 4;
     if (t0 >= nsamps) return;
-    if (t0 + 3 < nsamps) {
-        const float4 a = *reinterpret_cast<const float4 *>(x0 + t0);
-        float4 r;
-        r.x = a.x + (t0 + delta < nsamps ? x1[t0 + delta] : 0.0f);
-        r.y = a.y + (t0 + 1 + delta < nsamps ? x1[t0 + 1 + delta] : 0.0f);
-        r.z = a.z + (t0 + 2 + delta < nsamps ? x1[t0 + 2 + delta] : 0.0f);
-        r.w = a.w + (t0 + 3 + delta < nsamps ? x1[t0 + 3 + delta] : 0.0f);
-        *reinterpret_cast<float4 *>(o + t0) = r;
-    } else {
-        for (long long t = t0; t < nsamps; ++t) o[t] = x0[t] + (t + delta < nsamps ? x1[t + delta] : 0.0f);
+    float a[4], c[4 + 8];
+    const int span = 4 + nv - 1;                       // x1 samples t0 + dlo .. t0 + dlo + span - 1 serve every row (nv <= 9)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) a[i] = t0 + i < nsamps ? x0[t0 + i] : 0.0f;
+#pragma unroll
+    for (int i = 0; i < 12; ++i) c[i] = (i < span && t0 + dlo + i < nsamps) ? x1[t0 + dlo + i] : 0.0f;
+#pragma unroll
+    for (int v = 0; v < 9; ++v) {
+        if (v >= nv) break;
+        float *ov = o + (size_t)v * nsamps;
+        if (t0 + 3 < nsamps) {
+            *reinterpret_cast<float4 *>(ov + t0) = make_float4(a[0] + c[v], a[1] + c[v + 1], a[2] + c[v + 2], a[3] + c[v + 3]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (t0 + i < nsamps) ov[t0 + i] = a[i] + c[v + i];
+        }
     }
 }
 
@@ -491,10 +500,12 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
             const long long dl = dly(d, 2 * q + 1) - dly(d, 2 * q);
             lo = std::min(lo, dl); hi = std::max(hi, dl);
         }
-        if (lo < 0 || hi - lo > 64) return false;
-        ybase[q] = (int)h_ychan.size(); ylo[q] = (int)lo;
-        for (long long dl = lo; dl <= hi; ++dl) { h_ychan.push_back(2 * q); h_ydelta.push_back((int32_t)dl); }
+        if (lo < 0 || hi - lo > 8) return false;                    // the pre-sum kernel holds at most 9 rows of a pair
+        ybase[q] = (int)h_ydelta.size(); ylo[q] = (int)lo;
+        for (long long dl = lo; dl <= hi; ++dl) h_ydelta.push_back((int32_t)dl);
+        h_ychan.push_back(ybase[q]);                                 // first row of pair q (one more entry closes the list)
     }
+    h_ychan.push_back((int32_t)h_ydelta.size());
     const double f_lo = p->f_top + (p->nchans - 1) * p->foff;
     const double smax = 4.148808e3 * p->dm_step * (1.0 / (f_lo * f_lo) - 1.0 / (p->f_top * p->f_top)) / p->tsamp;
     h_sigma.resize(DB);
@@ -577,7 +588,7 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
     tt.dm_block = DB; tt.n_dm_blocks = nblk; tt.tile_t = TT;
     tt.max_off = worst;
     tt.sigma_max = *std::max_element(h_sigma.begin(), h_sigma.end());
-    tt.pairs = true; tt.nslab_max = nslab_max; tt.nyrows = (int)h_ychan.size();
+    tt.pairs = true; tt.nslab_max = nslab_max; tt.nyrows = (int)h_ydelta.size();
     return true;
 }
 
@@ -718,8 +729,8 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
                 MDSM_CUDA_TRY(cudaMalloc(&p->d_pairs, need));
                 p->pairs_bytes = need;
             }
-            dim3 grid((unsigned)((p->nsamps / 4 + 255) / 256), tt.nyrows, nb);
-            MDSM_REQUIRE(tt.nyrows <= 65535 && nb <= 65535, "pair pre-sum: grid too large");
+            dim3 grid((unsigned)((p->nsamps / 4 + 255) / 256), p->nchans / 2, nb);
+            MDSM_REQUIRE(p->nchans / 2 <= 65535 && nb <= 65535, "pair pre-sum: grid too large");
             pair_presum_kernel<<<grid, 256, 0, st>>>((const float *)d_in, (float *)p->d_pairs, tt.d_yrow_chan, tt.d_yrow_delta, beam0,
                                                      p->nchans, tt.nyrows, p->nsamps);
             MDSM_CUDA_TRY(cudaGetLastError());

@@ -154,6 +154,7 @@ struct TiledArgs {
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
     static constexpr bool kF32 = true, kTwoPhase = false;
+    static constexpr int PW = NW_ % 4 == 0 ? 4 : 1;     // producer warpgroup (register reallocation) or one producer warp
     using In = float; using Out = float; using Acc = unsigned long long;
     using Slab = SlabF32<D_, T_, NOFF_>;
     static_assert(T_ % 4 == 0 && (T_ / 4) % 2 == 1, "T/4 must be odd (bank-conflict-free 128-bit window loads)");
@@ -165,6 +166,7 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32P : Trait
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
     static constexpr bool kF32 = false, kTwoPhase = false;
+    static constexpr int PW = 1;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16<D_, T_, NOFF_>;
     static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
@@ -175,6 +177,7 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16P {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ + 1;
     static constexpr bool kF32 = false, kTwoPhase = true;
+    static constexpr int PW = 1;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16P<D_, T_, NOFF_>;
     static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
@@ -182,7 +185,7 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16P {
 
 // ------------------------------------------------------------------ the kernel
 template <typename Tr>
-__global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(const TiledArgs a)
+__global__ void __launch_bounds__((Tr::NW + Tr::PW) * 32, 1) dedisperse_tiled_kernel(const TiledArgs a)
 {
     using In = typename Tr::In;
     using Out = typename Tr::Out;
@@ -212,7 +215,10 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
     __syncthreads();
 
     const int ncp = a.nslab * CS;
-    if (warp == NW) {
+    if (warp >= NW) {
+        // NW % 4 == 0: the producer owns a whole warpgroup and hands its registers to the consumers
+        if constexpr (Tr::PW == 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (warp > NW) return;
         // ===== producer: lane r < CS copies row r of every slab, lane CS the slab's slice of the warp table =====
         if (lane > CS) return;
         int st = 0;
@@ -257,6 +263,7 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_tiled_kernel(
     }
 
     // ===== consumer warps =====
+    if constexpr (Tr::PW == 4) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
     Acc acc[D][AW];
     const uint32_t lane_base = smem_u32(smem) + lane * (T * (uint32_t)sizeof(In));
     const uint32_t tab_base = smem_u32(tabs) + warp * (CS * 8);
@@ -367,7 +374,7 @@ struct Geometry {
     int D, T, NW, CS, NOFF;
 };
 // compiled geometries; index = plan option "tiled_geom_<dtype>"
-constexpr Geometry kGeomF32[] = {{4, 28, 11, 16, 12}, {4, 20, 15, 8, 12}, {2, 28, 15, 16, 12}};   // last: coarse DM grids
+constexpr Geometry kGeomF32[] = {{4, 28, 11, 16, 12}, {4, 20, 15, 8, 12}, {2, 28, 15, 16, 12}, {4, 28, 12, 16, 12}};   // [2]: coarse DM grids; [3]: 12 warps (setmaxnreg), pair mode only
 constexpr Geometry kGeomU16[] = {{2, 40, 15, 16, 12}, {3, 40, 11, 8, 14}, {4, 40, 11, 8, 16}};   // index <= 1: two-phase rows
 constexpr int kNumGeomF32 = sizeof(kGeomF32) / sizeof(kGeomF32[0]);
 constexpr int kNumGeomU16 = sizeof(kGeomU16) / sizeof(kGeomU16[0]);
@@ -637,7 +644,7 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
     a.walk.ntile_t = (int)((p->nsamps_out + tt.sigma_max + tt.tile_t - 1) / tt.tile_t);
     a.walk.ntiles = (long long)a.walk.nblk * a.walk.ntile_t * nb;
     const int grid = (int)std::min<long long>(a.walk.ntiles, p->sm_count);
-    kern<<<grid, (Tr::NW + 1) * 32, smem, st>>>(a);
+    kern<<<grid, (Tr::NW + Tr::PW) * 32, smem, st>>>(a);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 1;
     return MDSM_OK;
@@ -676,19 +683,20 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
         std::vector<int32_t> rs, sig, src, nsl, yc, yd;
         std::vector<unsigned long long> tab;
         TiledTables &tt = p->tiled_f32;
-        if (build_tables_pairs(p, kGeomF32[0], tt, rs, tab, sig, src, nsl, yc, yd)) {
+        const int pg = p->tiled_geom_f32 == 1 ? 1 : (p->tiled_geom_f32 == 0 ? 0 : 3);   // pair mode is compiled for geometries 0, 1, 3 (default)
+        if (build_tables_pairs(p, kGeomF32[pg], tt, rs, tab, sig, src, nsl, yc, yd)) {
             if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig) ||
                 !upload(&tt.d_src_row, src) || !upload(&tt.d_nslab_blk, nsl) || !upload(&tt.d_yrow_chan, yc) || !upload(&tt.d_yrow_delta, yd)) {
                 mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
                 return MDSM_ECUDA;
             }
-            tt.geom = 0;
+            tt.geom = pg;
             tt.ok = true;
         }
     }
     if (p->nsamps % 4 == 0 && p->tiled_geom_f32 < kNumGeomF32)
-        for (int g = 0; g < kNumGeomF32 && !p->tiled_f32.ok; ++g) {
-            if (p->tiled_geom_f32 >= 0 && g != p->tiled_geom_f32) continue;
+        for (int g = 0; g < 3 && !p->tiled_f32.ok; ++g) {
+            if (p->tiled_geom_f32 >= 0 && p->tiled_geom_f32 < 3 && g != p->tiled_geom_f32) continue;
             const int rc = build_one(p, kGeomF32[g], 4, false, g, p->tiled_f32);
             if (rc != MDSM_OK) return rc;
         }
@@ -735,6 +743,8 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
                                                      p->nchans, tt.nyrows, p->nsamps);
             MDSM_CUDA_TRY(cudaGetLastError());
             p->launches += 1;
+            if (tt.geom == 1) return launch_tiled<GeomF32P<1>>(p, tt, p->d_pairs, beam0, nb, d_out, 0, st);
+            if (tt.geom == 3) return launch_tiled<GeomF32P<3>>(p, tt, p->d_pairs, beam0, nb, d_out, 0, st);
             return launch_tiled<GeomF32P<0>>(p, tt, p->d_pairs, beam0, nb, d_out, 0, st);
         }
         switch (tt.geom) {

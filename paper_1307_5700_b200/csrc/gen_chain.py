@@ -194,7 +194,7 @@ def gen_f32p(D, T, NOFF):
     e = Emit()
     e("{")
     e(f".reg .b64 w<{W2}>;")
-    e(".reg .b32 lo, hi, p, tp, tm;")
+    e(".reg .b32 lo, hi, nlo, nhi, p, tp, tm;")
     e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3, s0, s1, s2, s3;")
     e(".reg .f32 a0, a1, x0, x1, y0, y1;")
 
@@ -209,8 +209,9 @@ def gen_f32p(D, T, NOFF):
     e("bra.uni HEAD;")
     e("TAIL:")
     e("@pl bra.uni Bend;")
-    e("add.u32 tp, tp, 8; ld.shared.v2.b32 {lo, hi}, [tp];")
+    e("add.u32 tp, tp, 8; mov.b32 lo, nlo; mov.b32 hi, nhi;")
     e("HEAD:")
+    e("ld.shared.v2.b32 {nlo, nhi}, [tp+8];")                       # the entry after this one (unused after the last row)
     e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
     for i in range(NCH - base_ch):
         e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
@@ -426,7 +427,7 @@ def gen_u16p(D, T, NOFF):
 F32_VARIANTS = [(4, 28, 12), (4, 20, 12), (2, 28, 12)]
 U16_VARIANTS = [(4, 40, 16)]
 U16P_VARIANTS = [(2, 40, 12), (3, 40, 14)]
-F32P_VARIANTS = [(4, 28, 12)]
+F32P_VARIANTS = [(4, 28, 12), (4, 20, 12)]
 
 
 def main(out):

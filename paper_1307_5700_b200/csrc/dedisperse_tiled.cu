@@ -153,7 +153,7 @@ struct TiledArgs {
 
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
-    static constexpr bool kF32 = true, kTwoPhase = false;
+    static constexpr bool kF32 = true, kTwoPhase = false, kPairs = false;
     static constexpr int PW = NW_ % 4 == 0 ? 4 : 1;     // producer warpgroup (register reallocation) or one producer warp
     using In = float; using Out = float; using Acc = unsigned long long;
     using Slab = SlabF32<D_, T_, NOFF_>;
@@ -161,11 +161,12 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32 {
 };
 // pair pre-sum mode: same data types as TraitsF32, loop with skip bits and per-slot dispatchers (gen_chain.py: gen_f32p)
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsF32P : TraitsF32<D_, T_, NW_, CS_, NOFF_> {
+    static constexpr bool kPairs = true;
     using Slab = SlabF32P<D_, T_, NOFF_>;
 };
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ / 2;
-    static constexpr bool kF32 = false, kTwoPhase = false;
+    static constexpr bool kF32 = false, kTwoPhase = false, kPairs = false;
     static constexpr int PW = 1;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16<D_, T_, NOFF_>;
@@ -176,7 +177,7 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16 {
 // outputs shifted by one sample), no shifted window copy (gen_chain.py: gen_u16p)
 template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16P {
     static constexpr int D = D_, T = T_, NW = NW_, CS = CS_, AW = T_ + 1;
-    static constexpr bool kF32 = false, kTwoPhase = true;
+    static constexpr bool kF32 = false, kTwoPhase = true, kPairs = false;
     static constexpr int PW = 1;
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16P<D_, T_, NOFF_>;
@@ -230,14 +231,14 @@ __global__ void __launch_bounds__((Tr::NW + Tr::PW) * 32, 1) dedisperse_tiled_ke
             const long long tile_t0 = (long long)tt * (32 * T);
             const In *beam_in = reinterpret_cast<const In *>(a.in) + (size_t)(a.beam0 + bb) * a.nrows_src * (size_t)a.nsamps;
             const int32_t *rs = a.row_start + (size_t)blk * ncp;
-            const int32_t *sr = a.src_row ? a.src_row + (size_t)blk * ncp : nullptr;
+            const int32_t *sr = Tr::kPairs ? a.src_row + (size_t)blk * ncp : nullptr;
             const unsigned long long *wt = a.warp_tab + (size_t)blk * a.nslab * NW * CS;
-            const int nslab_b = a.nslab_blk ? a.nslab_blk[blk] : a.nslab;
+            const int nslab_b = Tr::kPairs ? a.nslab_blk[blk] : a.nslab;
             for (int slab = 0; slab < nslab_b; ++slab) {
                 if (!first_lap) mbar_wait_sleep(&empty[st], ph);
                 if (lane < CS) {
                     const int r = slab * CS + lane;
-                    const int c = sr ? sr[r] : (r < a.nchans ? r : -1);      // source row of staged row r
+                    const int c = Tr::kPairs ? sr[r] : (r < a.nchans ? r : -1);      // source row of staged row r
                     uint32_t bytes = 0;
                     long long lo = 0, g0 = 0;
                     if (c >= 0) {
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__((Tr::NW + Tr::PW) * 32, 1) dedisperse_tiled_ke
         const long long tile_t0 = (long long)tt * (32 * T);
         const int b = a.beam0 + bb;
 #pragma unroll 1
-        const int nslab_b = a.nslab_blk ? a.nslab_blk[blk] : a.nslab;
+        const int nslab_b = Tr::kPairs ? a.nslab_blk[blk] : a.nslab;
 #pragma unroll 1
         for (int s0 = 0; s0 < nslab_b; s0 += a.slabs_per_part) {
 #pragma unroll

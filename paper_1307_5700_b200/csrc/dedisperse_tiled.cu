@@ -735,7 +735,18 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
                 cudaFree(p->d_pairs);
                 p->d_pairs = nullptr;
                 p->pairs_bytes = 0;
-                MDSM_CUDA_TRY(cudaMalloc(&p->d_pairs, need));
+                if (cudaMalloc(&p->d_pairs, need) != cudaSuccess) {
+                    // no room for the pre-summed copy: this plan goes on without pair pre-sums (tables rebuilt once;
+                    // the caller's stream may still run kernels of this plan, so wait for them before freeing tables)
+                    (void)cudaGetLastError();
+                    p->d_pairs = nullptr;
+                    p->pair_presum = 0;
+                    MDSM_CUDA_TRY(cudaDeviceSynchronize());
+                    const int rc = mdsm_tiled_build_tables(p);
+                    if (rc != MDSM_OK) return rc;
+                    if (!p->tiled_f32.ok) return mdsm_launch_dedisperse_direct(p, d_in, dtype, beam0, nb, d_out, st);
+                    return mdsm_launch_dedisperse_tiled(p, d_in, dtype, beam0, nb, d_out, st);
+                }
                 p->pairs_bytes = need;
             }
             dim3 grid((unsigned)((p->nsamps / 4 + 255) / 256), p->nchans / 2, nb);

@@ -124,3 +124,31 @@ def test_fp32_same_sign_data_stays_inside_the_tolerance_at_4096_channels():
             got = out_to_numpy(p.dedisperse(torch.from_numpy(x).cuda(), kernel=2), p.nsamps_out)
         ratio = np.abs(got.astype(np.float64) - ref) / (1e-5 * ab + 1e-6)
         assert ratio.max() < 0.7, ratio.max()              # measured 0.42 / 0.44: a factor two of margin
+
+
+def test_pair_presum_falls_back_when_its_scratch_does_not_fit():
+    """With device memory nearly full the fp32 path must go on without the pre-summed copy, not fail."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    args = (1, 256, 418.0, -20.0 / 256, 51.2e-6, 1 << 17, 0.0, 0.1, 64)         # pair scratch ~ 2 x 134 MB
+    g = np.random.default_rng(12)
+    x = g.normal(size=(1, 256, 1 << 17)).astype(np.float32)
+    d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
+    ref, ab = oracle.dedisperse(x, d)
+    with Plan(args) as p:
+        dx = torch.from_numpy(x).cuda()
+        out = torch.full((1, 64, 1 << 17), -7, dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        torch.cuda.empty_cache()
+        free, _ = torch.cuda.mem_get_info()
+        hog = torch.empty((max(free - (96 << 20), 0),), dtype=torch.uint8, device="cuda")   # leave 96 MB
+        try:
+            l0 = m.mdsm_plan_launch_count(p.h)
+            m.mdsm_dedisperse(p.h, dx, 0, 1, out)
+            torch.cuda.synchronize()
+            assert m.mdsm_plan_launch_count(p.h) - l0 == 1                      # no pre-pass launch: plain tiled kernel
+        finally:
+            del hog
+            torch.cuda.empty_cache()
+        got = out_to_numpy(out, p.nsamps_out)
+        assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)

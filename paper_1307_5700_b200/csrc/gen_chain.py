@@ -181,7 +181,8 @@ def gen_f32p(D, T, NOFF):
     """fp32 loop of the pair pre-sum mode: a staged row is used by a SUBSET of the warp's DMs (bit 7 of a DM's offset
     byte = "skips this row").  The chain hops from one participating DM to the next: after its adds a block tests the
     skip bits of the DMs behind it (one predicated branch each) and enters the shared dispatcher DISP_j' of the first
-    participant, or the loop tail when none is left.  One loop head (not copied), one dispatcher per DM slot."""
+    participant, or the loop tail when none is left.  One loop head (not copied), one dispatcher per DM slot; a block
+    dispatches the NEXT slot itself when that slot uses the row (half of the time: one taken branch less)."""
     assert T % 4 == 0 and D <= 4
     A2 = T // 2
     NCH = nchunks(T, NOFF, 4)
@@ -226,10 +227,17 @@ def gen_f32p(D, T, NOFF):
         tree_bits(e, j)
         tree_branch(e, j, NOFF)
         tree_stubs(e, j, NOFF)
+        if j + 1 < D:
+            e(f"HOP{j}:")                      # slot j+1 skips the row: look further (rare enough to share the code)
+            skip_preds(j + 2)
+            hop(j + 2)
         for k in range(NOFF):
             m = k // 2
             e(f"B{j}_{k}:")
-            skip_preds(j + 1)
+            if j + 1 < D:
+                skip_preds_one = f"and.b32 tm, hi, {0x80 << (8 * (j + 1))}; setp.ne.u32 s{j + 1}, tm, 0;"
+                e(skip_preds_one)
+                tree_bits(e, j + 1)
             body = ""
             for i in range(A2):
                 a = j * A2 + i
@@ -239,7 +247,11 @@ def gen_f32p(D, T, NOFF):
                     body += (f"mov.b64 {{a0,a1}}, %{a}; mov.b64 {{x0,x1}}, w{m + i}; mov.b64 {{y0,y1}}, w{m + i + 1}; "
                              f"add.f32 a0, a0, x1; add.f32 a1, a1, y0; mov.b64 %{a}, {{a0,a1}}; ")
             e(body)
-            hop(j + 1)
+            if j + 1 < D:
+                e(f"@s{j + 1} bra.uni HOP{j};")
+                tree_branch(e, j + 1, NOFF)     # the next slot uses the row: dispatch it from here (one taken branch less)
+            else:
+                e("bra.uni TAIL;")
     e("Bend:")
     e("}")
     s = [f"// f32x2 slab loop, pair pre-sum mode: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]

@@ -338,7 +338,7 @@ def main():
     adds = float(cfg.nchans) * cfg.nbeams * cfg.ndms * nso          # algorithmic adds per launch
     hbm_bytes = x.nbytes + 4.0 * cfg.nbeams * cfg.ndms * nso
     hbm_peak = measured_hbm_peak()
-    roofline = {"bound": "alu", "kernel": "dedisperse", "achieved": adds / dd / 1e9, "peak": peak / 1e9, "unit": "Gadd/s",
+    roofline = {"bound": "alu", "kernel": "dedisperse (mdsm_dedisperse call: pre-pass or widening kernel + tiled kernel, timed together)", "achieved": adds / dd / 1e9, "peak": peak / 1e9, "unit": "Gadd/s",
                 "frac": adds / dd / peak, "peak_source": "measured in this run: mdsm_measure_add_peak (register-only add loop, all SMs)",
                 "peak_nominal": NOMINAL_ADD_PEAK / 1e9, "measured_peaks_gadd_s": {k: v / 1e9 for k, v in peaks.items()},
                 "ms_per_launch": dd * 1e3, "hbm_floor_ms": 1e3 * hbm_bytes / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),

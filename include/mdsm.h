@@ -88,7 +88,13 @@ int mdsm_rfi_clip(mdsm_plan *plan, void *d_in, int dtype, int beam0, int nb,
 /* Brute-force incoherent dedispersion:
  *   out[b][d][t] = sum_c in[b][c][t + delay(d,c)],   t in [0, nsamps_out)
  * MDSM_F32: float in, float out (fp32 accumulation; |err| <= 1e-5 * sum_c|in| + 1e-6).
- * MDSM_U8 : uint8 in, uint32 out, exact. */
+ * MDSM_U8 : uint8 in, uint32 out, exact.
+ * d_in [nbeams][nchans][nsamps], d_out [nbeams][ndms][nsamps] (only t < nsamps_out of the rows of beams
+ * [beam0, beam0+nb) is written), both caller-owned device buffers; 16-byte aligned buffers and nsamps % 4 == 0
+ * (uint8: % 8) take the tiled kernels, anything else the direct kernel.  Asynchronous on cuda_stream.  The FIRST call
+ * of a dtype allocates plan-owned scratch (uint8: a uint16 copy of the input; float: the pre-summed channel pairs,
+ * about two input sizes -- if that does not fit, the plan synchronises the device once, drops the pair pre-sums and
+ * goes on with the plain tiled kernel); later calls allocate nothing. */
 int mdsm_dedisperse(mdsm_plan *plan, const void *d_in, int dtype, int beam0, int nb,
                     void *d_out, void *cuda_stream);
 

@@ -205,7 +205,7 @@ def main():
     plan = m.mdsm_plan_create(*cfg.plan_args())
     m.mdsm_plan_set_option(plan, "dedisp_kernel", args.kernel)
     if args.pairs >= 0:
-        m.mdsm_plan_set_option(plan, "pair_presum", args.pairs)
+        m.mdsm_plan_set_option(plan, "pair_presum_u8" if cfg.dtype == "u8" else "pair_presum", args.pairs)
     if args.geom >= 0:
         m.mdsm_plan_set_option(plan, "tiled_geom_" + cfg.dtype, args.geom)
     nso = m.mdsm_plan_nsamps_out(plan)

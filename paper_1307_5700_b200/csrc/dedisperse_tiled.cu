@@ -145,6 +145,7 @@ struct TiledArgs {
     const int32_t *src_row;               // pair mode: [nblk][nslab*CS] source row of staged row r (-1: none); else nullptr
     const int32_t *nslab_blk;             // pair mode: [nblk] slabs of the block; else nullptr
     int nrows_src;                        // rows per beam of the staged source (nchans, or the pre-summed copy's row count)
+    int nparts;                           // pair mode: parts per tile (slabs per part = the block's slabs / nparts); else 0
     int beam0, nchans, nslab, slabs_per_part, ndms;
     long long nsamps, nsamps_out;
     int row_elems, stages;
@@ -182,6 +183,12 @@ template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16P {
     using In = uint16_t; using Out = uint32_t; using Acc = unsigned;
     using Slab = SlabU16P<D_, T_, NOFF_>;
     static_assert(T_ % 8 == 0 && (T_ / 8) % 2 == 1, "T/8 must be odd (bank-conflict-free 128-bit window loads)");
+};
+
+// integer pair pre-sum mode: TraitsU16P's data layout, loop with skip bits (gen_chain.py: gen_u16pp)
+template <int D_, int T_, int NW_, int CS_, int NOFF_> struct TraitsU16PP : TraitsU16P<D_, T_, NW_, CS_, NOFF_> {
+    static constexpr bool kPairs = true;
+    using Slab = SlabU16PP<D_, T_, NOFF_>;
 };
 
 // ------------------------------------------------------------------ the kernel
@@ -277,13 +284,14 @@ __global__ void __launch_bounds__((Tr::NW + Tr::PW) * 32, 1) dedisperse_tiled_ke
         const int b = a.beam0 + bb;
 #pragma unroll 1
         const int nslab_b = Tr::kPairs ? a.nslab_blk[blk] : a.nslab;
+        const int spp = Tr::kPairs ? nslab_b / a.nparts : a.slabs_per_part;
 #pragma unroll 1
-        for (int s0 = 0; s0 < nslab_b; s0 += a.slabs_per_part) {
+        for (int s0 = 0; s0 < nslab_b; s0 += spp) {
 #pragma unroll
             for (int j = 0; j < D; ++j)
 #pragma unroll
                 for (int i = 0; i < AW; ++i) acc[j][i] = 0;      // (+0.f, +0.f) / (0, 0)
-            const int s1 = min(nslab_b, s0 + a.slabs_per_part);
+            const int s1 = min(nslab_b, s0 + spp);
 #pragma unroll 1
             for (int slab = s0; slab < s1; ++slab) {
                 mbar_wait(&full[st], ph);
@@ -367,6 +375,38 @@ __global__ void __launch_bounds__(256) pair_presum_kernel(const float *__restric
             for (int i = 0; i < 4; ++i)
                 if (t0 + i < nsamps) ov[t0 + i] = a[i] + c[v + i];
         }
+    }
+}
+
+// the same for the integer path: uint8 in, uint16 sums out (<= 510), so the widening pass is not needed in pair mode
+__global__ void __launch_bounds__(256) pair_presum_u8_kernel(const uint8_t *__restrict__ in, uint16_t *__restrict__ y,
+                                                             const int32_t *__restrict__ pair_row0, const int32_t *__restrict__ yrow_delta,
+                                                             int beam0, int nchans, int nyrows, long long nsamps)
+{
+    const int q = blockIdx.y, b = beam0 + blockIdx.z;
+    const int row0 = pair_row0[q], nv = pair_row0[q + 1] - row0;
+    const int dlo = yrow_delta[row0];
+    const uint8_t *x0 = in + ((size_t)b * nchans + 2 * q) * (size_t)nsamps;
+    const uint8_t *x1 = x0 + nsamps;
+    uint16_t *o = y + ((size_t)b * nyrows + row0) * (size_t)nsamps;
+    const long long t0 = ((long long)blockIdx.x * 256 + threadIdx.x) * 8;           // nsamps % 8 == 0 on this path
+    if (t0 >= nsamps) return;
+    unsigned a[8], c[8 + 8];
+    const uint2 av = *reinterpret_cast<const uint2 *>(x0 + t0);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = ((i < 4 ? av.x : av.y) >> (8 * (i & 3))) & 0xffu;
+    const int span = 8 + nv - 1;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = (i < span && t0 + dlo + i < nsamps) ? x1[t0 + dlo + i] : 0u;
+#pragma unroll
+    for (int v = 0; v < 9; ++v) {
+        if (v >= nv) break;
+        uint4 r;
+        r.x = (a[0] + c[v]) | ((a[1] + c[v + 1]) << 16);
+        r.y = (a[2] + c[v + 2]) | ((a[3] + c[v + 3]) << 16);
+        r.z = (a[4] + c[v + 4]) | ((a[5] + c[v + 5]) << 16);
+        r.w = (a[6] + c[v + 6]) | ((a[7] + c[v + 7]) << 16);
+        *reinterpret_cast<uint4 *>(o + (size_t)v * nsamps + t0) = r;
     }
 }
 
@@ -491,12 +531,17 @@ static bool build_tables(const mdsm_plan *p, const Geometry &g, int al, bool two
 // Pair mode tables: the rows a DM block stages are (channel pair, delay difference) rows of the pre-summed copy; a row
 // is used by the DMs of the block whose delay difference for that pair equals the row's, the others carry offset 15
 // (= skip) in the window entry.  Same geometry, shear and entry format as build_tables.
-static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTables &tt, std::vector<int32_t> &h_rs,
+// al = samples per 16 bytes of the staged element; two_phase = dispatch index 8*(o & 1) + (o >> 1) (integer kernel);
+// part_pairs > 0: the rows are grouped in parts of that many pairs (16-bit lane capacity), every part of a block padded
+// with unused rows to the same number of whole slabs.
+static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, int al, bool two_phase, int part_pairs, TiledTables &tt, std::vector<int32_t> &h_rs,
                                std::vector<unsigned long long> &h_tab, std::vector<int32_t> &h_sigma, std::vector<int32_t> &h_src,
                                std::vector<int32_t> &h_nslab, std::vector<int32_t> &h_ychan, std::vector<int32_t> &h_ydelta)
 {
     if (p->nchans % 2 || p->nchans < 2 || g.NOFF > 15) return false;
-    const int al = 4, DB = g.D * g.NW, TT = 32 * g.T, np = p->nchans / 2;
+    const int DB = g.D * g.NW, TT = 32 * g.T, np = p->nchans / 2, esize = 16 / al;
+    const int nparts = part_pairs > 0 ? (np + part_pairs - 1) / part_pairs : 1;
+    if (part_pairs <= 0) part_pairs = np;
     const int nblk = (p->ndms + DB - 1) / DB;
     auto dly = [&](int d, int c) { return (long long)p->h_delay[(size_t)std::min(d, p->ndms - 1) * p->nchans + c]; };
     // rows of the pre-summed copy: every delay difference a pair takes over the whole DM grid
@@ -519,11 +564,13 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
     h_sigma.resize(DB);
     for (int dl = 0; dl < DB; ++dl) h_sigma[dl] = (int32_t)llround(0.5 * smax * dl);
     // per block: the list of (pair, delta) rows some DM of the block uses
-    struct Row { int q, delta; };
+    struct Row { int q, delta; };                 // q < 0: padding row nobody uses
     std::vector<std::vector<Row>> rows(nblk);
     int nslab_max = 0;
     h_nslab.resize(nblk);
     for (int blk = 0; blk < nblk; ++blk) {
+        std::vector<std::vector<Row>> part(nparts);
+        size_t longest = 0;
         for (int q = 0; q < np; ++q) {
             std::vector<int> seen;
             for (int dl = 0; dl < DB; ++dl) {
@@ -532,9 +579,15 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
                 if (std::find(seen.begin(), seen.end(), de) == seen.end()) seen.push_back(de);
             }
             std::sort(seen.begin(), seen.end());
-            for (int de : seen) rows[blk].push_back({q, de});
+            for (int de : seen) part[q / part_pairs].push_back({q, de});
         }
-        h_nslab[blk] = ((int)rows[blk].size() + g.CS - 1) / g.CS;
+        for (auto &pr : part) longest = std::max(longest, pr.size());
+        const int spp = ((int)longest + g.CS - 1) / g.CS;                  // slabs per part of this block
+        for (auto &pr : part) {
+            if (nparts > 1) pr.resize((size_t)spp * g.CS, Row{-1, 0});       // a single part may end with a ragged slab
+            rows[blk].insert(rows[blk].end(), pr.begin(), pr.end());
+        }
+        h_nslab[blk] = spp * nparts;
         nslab_max = std::max(nslab_max, h_nslab[blk]);
     }
     const int ncp = nslab_max * g.CS;
@@ -542,21 +595,21 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
     h_src.assign((size_t)nblk * ncp, -1);
     h_tab.assign((size_t)nblk * nslab_max * g.NW * g.CS, 0ULL);
     auto e_of = [&](int blk, int dl, int c) { return dly(blk * DB + dl, c) - h_sigma[dl]; };
-    auto uses = [&](int blk, int dl, const Row &r) { const int d = blk * DB + dl; return dly(d, 2 * r.q + 1) - dly(d, 2 * r.q) == r.delta; };
+    auto uses = [&](int blk, int dl, const Row &r) { const int d = blk * DB + dl; return r.q >= 0 && dly(d, 2 * r.q + 1) - dly(d, 2 * r.q) == r.delta; };
     long long max_need = 0;
     int worst = 0;
     for (int pass = 0; pass < 2; ++pass) {
         const int row_elems = (int)((max_need + al - 1) / al * al);
-        if (pass == 1 && (worst >= g.NOFF || (long long)g.CS * row_elems * 4 >= (1 << 18))) return false;
+        if (pass == 1 && (worst >= g.NOFF || (long long)g.CS * row_elems * esize >= (1 << 18))) return false;
         for (int blk = 0; blk < nblk; ++blk)
             for (int ri = 0; ri < (int)rows[blk].size(); ++ri) {
                 const Row &r = rows[blk][ri];
-                const int c = 2 * r.q;
+                const int c = r.q >= 0 ? 2 * r.q : 0;
                 long long mn = 1LL << 60;
                 for (int dl = 0; dl < DB; ++dl)
                     if (uses(blk, dl, r)) mn = std::min(mn, e_of(blk, dl, c));
-                const long long rs = floor_to(mn, al);
-                if (pass == 1) {
+                const long long rs = r.q >= 0 ? floor_to(mn, al) : 0;
+                if (pass == 1 && r.q >= 0) {
                     h_rs[(size_t)blk * ncp + ri] = (int32_t)rs;
                     h_src[(size_t)blk * ncp + ri] = ybase[r.q] + (r.delta - ylo[r.q]);
                 }
@@ -580,11 +633,14 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
                         }
                         continue;
                     }
-                    unsigned long long lo = (unsigned long long)(((long long)rr * row_elems + A) * 4);
+                    unsigned long long lo = (unsigned long long)(((long long)rr * row_elems + A) * esize);
                     for (int i = 0; i < chunks - g.T / al; ++i) lo |= 1ULL << (28 + i);
                     if (last) lo |= 1ULL << 31;
                     unsigned long long hi = 0;
-                    for (int j = 0; j < g.D; ++j) hi |= (unsigned long long)(use[j] ? (e[j] - A) : 0x80) << (8 * j);   // bit 7: skips the row
+                    for (int j = 0; j < g.D; ++j) {
+                        const unsigned long long o = (unsigned long long)(e[j] - A);
+                        hi |= (use[j] ? (two_phase ? 8 * (o & 1) + (o >> 1) : o) : 0x80ULL) << (8 * j);     // bit 7: skips the row
+                    }
                     h_tab[(((size_t)blk * nslab_max + slab) * g.NW + w) * g.CS + rr] = lo | (hi << 32);
                 }
             }
@@ -596,7 +652,7 @@ static bool build_tables_pairs(const mdsm_plan *p, const Geometry &g, TiledTable
     tt.dm_block = DB; tt.n_dm_blocks = nblk; tt.tile_t = TT;
     tt.max_off = worst;
     tt.sigma_max = *std::max_element(h_sigma.begin(), h_sigma.end());
-    tt.pairs = true; tt.nslab_max = nslab_max; tt.nyrows = (int)h_ydelta.size();
+    tt.pairs = true; tt.nslab_max = nslab_max; tt.nyrows = (int)h_ydelta.size(); tt.nparts = nparts;
     return true;
 }
 
@@ -637,6 +693,7 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
     a.src_row = tt.pairs ? tt.d_src_row : nullptr;
     a.nslab_blk = tt.pairs ? tt.d_nslab_blk : nullptr;
     a.nrows_src = tt.pairs ? tt.nyrows : p->nchans;
+    a.nparts = tt.pairs ? tt.nparts : 0;
     a.beam0 = beam0; a.nchans = p->nchans; a.nslab = tt.pairs ? tt.nslab_max : nslab; a.ndms = p->ndms;
     a.slabs_per_part = part_chans > 0 ? part_chans / Tr::CS : (tt.pairs ? tt.nslab_max : nslab);
     a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out;
@@ -654,6 +711,7 @@ static int launch_tiled(mdsm_plan *p, const TiledTables &tt, const void *d_in, i
 template <int G> using GeomF32 = TraitsF32<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
 template <int G> using GeomF32P = TraitsF32P<kGeomF32[G].D, kGeomF32[G].T, kGeomF32[G].NW, kGeomF32[G].CS, kGeomF32[G].NOFF>;
 template <int G> using GeomU16 = TraitsU16<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
+template <int G> using GeomU16PP = TraitsU16PP<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
 template <int G> using GeomU16P = TraitsU16P<kGeomU16[G].D, kGeomU16[G].T, kGeomU16[G].NW, kGeomU16[G].CS, kGeomU16[G].NOFF>;
 
 static int build_one(mdsm_plan *p, const Geometry &g, int al, bool two_phase, int geom, TiledTables &tt)
@@ -685,7 +743,7 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
         std::vector<unsigned long long> tab;
         TiledTables &tt = p->tiled_f32;
         const int pg = p->tiled_geom_f32 == 1 ? 1 : (p->tiled_geom_f32 == 0 ? 0 : 3);   // pair mode is compiled for geometries 0, 1, 3 (default)
-        if (build_tables_pairs(p, kGeomF32[pg], tt, rs, tab, sig, src, nsl, yc, yd)) {
+        if (build_tables_pairs(p, kGeomF32[pg], 4, false, 0, tt, rs, tab, sig, src, nsl, yc, yd)) {
             if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig) ||
                 !upload(&tt.d_src_row, src) || !upload(&tt.d_nslab_blk, nsl) || !upload(&tt.d_yrow_chan, yc) || !upload(&tt.d_yrow_delta, yd)) {
                 mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -701,6 +759,20 @@ int mdsm_tiled_build_tables(mdsm_plan *p)
             const int rc = build_one(p, kGeomF32[g], 4, false, g, p->tiled_f32);
             if (rc != MDSM_OK) return rc;
         }
+    if (p->pair_presum_u8 && p->nsamps % 8 == 0 && p->tiled_geom_u8 <= 0) {
+        std::vector<int32_t> rs, sig, src, nsl, yc, yd;
+        std::vector<unsigned long long> tab;
+        TiledTables &tt = p->tiled_u8;
+        if (build_tables_pairs(p, kGeomU16[0], 8, true, kPartChansU16 / 2, tt, rs, tab, sig, src, nsl, yc, yd)) {
+            if (!upload(&tt.d_row_start, rs) || !upload((unsigned long long **)&tt.d_warp_tab, tab) || !upload(&tt.d_sigma, sig) ||
+                !upload(&tt.d_src_row, src) || !upload(&tt.d_nslab_blk, nsl) || !upload(&tt.d_yrow_chan, yc) || !upload(&tt.d_yrow_delta, yd)) {
+                mdsm_set_error("tiled table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+                return MDSM_ECUDA;
+            }
+            tt.geom = 0;
+            tt.ok = true;
+        }
+    }
     if (p->nsamps % 8 == 0 && p->tiled_geom_u8 < kNumGeomU16)
         for (int g = 0; g < kNumGeomU16 && !p->tiled_u8.ok; ++g) {
             if (p->tiled_geom_u8 >= 0 && g != p->tiled_geom_u8) continue;
@@ -770,6 +842,33 @@ int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int 
     // uint8: widen the beams of this call to uint16 in the plan's scratch (allocated on first use, whole plan)
     const TiledTables &tt = p->tiled_u8;
     const size_t beam_elems = (size_t)p->nchans * (size_t)p->nsamps;
+    if (tt.pairs) {
+        // pair mode: the pre-pass writes uint16 pair sums (which also widens), the tiled kernel walks its rows
+        const size_t needp = (size_t)p->nbeams * tt.nyrows * (size_t)p->nsamps * sizeof(uint16_t);
+        if (p->widen_bytes < needp) {
+            cudaFree(p->d_widen);
+            p->d_widen = nullptr;
+            p->widen_bytes = 0;
+            if (cudaMalloc(&p->d_widen, needp) != cudaSuccess) {
+                (void)cudaGetLastError();
+                p->d_widen = nullptr;
+                p->pair_presum_u8 = 0;                       // no room: go on without pair pre-sums (see the fp32 path)
+                MDSM_CUDA_TRY(cudaDeviceSynchronize());
+                const int rc = mdsm_tiled_build_tables(p);
+                if (rc != MDSM_OK) return rc;
+                if (!p->tiled_u8.ok) return mdsm_launch_dedisperse_direct(p, d_in, dtype, beam0, nb, d_out, st);
+                return mdsm_launch_dedisperse_tiled(p, d_in, dtype, beam0, nb, d_out, st);
+            }
+            p->widen_bytes = needp;
+        }
+        dim3 grid((unsigned)((p->nsamps / 8 + 255) / 256), p->nchans / 2, nb);
+        MDSM_REQUIRE(p->nchans / 2 <= 65535 && nb <= 65535, "pair pre-sum: grid too large");
+        pair_presum_u8_kernel<<<grid, 256, 0, st>>>((const uint8_t *)d_in, (uint16_t *)p->d_widen, tt.d_yrow_chan, tt.d_yrow_delta, beam0,
+                                                    p->nchans, tt.nyrows, p->nsamps);
+        MDSM_CUDA_TRY(cudaGetLastError());
+        p->launches += 1;
+        return launch_tiled<GeomU16PP<0>>(p, tt, p->d_widen, beam0, nb, d_out, 0, st);
+    }
     const size_t need = (size_t)p->nbeams * beam_elems * sizeof(uint16_t);
     if (p->widen_bytes < need) {
         cudaFree(p->d_widen);

@@ -435,11 +435,100 @@ def gen_u16p(D, T, NOFF):
     return "\n".join(s)
 
 
+def gen_u16pp(D, T, NOFF):
+    """Two-phase u16x2 loop of the pair pre-sum mode: gen_u16p's add blocks (dispatch index = 8*(o & 1) + (o >> 1)) with
+    gen_f32p's control flow (bit 7 of a DM's byte = the DM skips the row; hops, one dispatcher per DM slot, the next
+    slot dispatched from inside the block when it uses the row)."""
+    assert T % 8 == 0 and D <= 4 and NOFF <= 16
+    A = T // 2
+    AW = 2 * A + 1
+    NCH = nchunks(T, NOFF, 8)
+    WE = NCH * 4
+    base_ch = T // 8
+    assert NCH - base_ch <= 3
+    nacc = D * AW
+    SB, TAB = nacc, nacc + 1
+    name = f"slab_u16pp_{D}_{T}_{NOFF}"
+    e = Emit()
+    e("{")
+    e(f".reg .b32 we<{WE}>;")
+    e(".reg .b32 lo, hi, nlo, nhi, p, tp, tm;")
+    e(".reg .pred q0, q1, q2, pl, b0, b1, b2, b3, s0, s1, s2, s3;")
+
+    def skip_preds(first):
+        for j in range(first, D):
+            e(f"and.b32 tm, hi, {0x80 << (8 * j)}; setp.ne.u32 s{j}, tm, 0;")
+
+    def hop(first):
+        e(" ".join(f"@!s{j} bra.uni DISP{j};" for j in range(first, D)) + " bra.uni TAIL;")
+
+    e(f"mov.u32 tp, %{TAB}; ld.shared.v2.b32 {{lo, hi}}, [tp];")
+    e("bra.uni HEAD;")
+    e("TAIL:")
+    e("@pl bra.uni Bend;")
+    e("add.u32 tp, tp, 8; mov.b32 lo, nlo; mov.b32 hi, nhi;")
+    e("HEAD:")
+    e("ld.shared.v2.b32 {nlo, nhi}, [tp+8];")
+    e("and.b32 p, lo, 0x3ffff; add.u32 p, p, %" + str(SB) + ";")
+    for i in range(NCH - base_ch):
+        e(f"and.b32 tm, lo, {1 << (28 + i)}; setp.ne.u32 q{i}, tm, 0;")
+    e("setp.lt.s32 pl, lo, 0;")
+    skip_preds(0)
+    for i in range(NCH):
+        pred = f"@q{i - base_ch} " if i >= base_ch else ""
+        e(f"{pred}ld.shared.v4.b32 {{we{4 * i}, we{4 * i + 1}, we{4 * i + 2}, we{4 * i + 3}}}, [p+{16 * i}];")
+    hop(0)
+    for j in range(D):
+        e(f"DISP{j}:")
+        tree_bits(e, j)
+        tree_branch(e, j, 16)
+        tree_stubs(e, j, 16)
+        if j + 1 < D:
+            e(f"HOP{j}:")
+            skip_preds(j + 2)
+            hop(j + 2)
+        for idx in range(16):
+            odd, m = idx // 8, idx % 8
+            e(f"B{j}_{idx}:")
+            if 2 * m + odd >= NOFF:
+                e("bra.uni Bend;")
+                continue
+            if j + 1 < D:
+                e(f"and.b32 tm, hi, {0x80 << (8 * (j + 1))}; setp.ne.u32 s{j + 1}, tm, 0;")
+                tree_bits(e, j + 1)
+            body = ""
+            n = A + 1 if odd else A
+            for i in range(n):
+                a = j * AW + (A + i if odd else i)
+                if i % 2 == 0:
+                    body += f"add.u32 %{a}, %{a}, we{m + i}; "
+                else:
+                    body += f"mad.lo.u32 %{a}, we{m + i}, 1, %{a}; "
+            e(body)
+            if j + 1 < D:
+                e(f"@s{j + 1} bra.uni HOP{j};")
+                tree_branch(e, j + 1, 16)
+            else:
+                e("bra.uni TAIL;")
+    e("Bend:")
+    e("}")
+    s = [f"// two-phase u16x2 slab loop, pair pre-sum mode: D={D} DMs x T={T} samples, offsets < {NOFF}, {NCH} window chunks"]
+    s.append(f"__device__ __forceinline__ void {name}(unsigned (&acc)[{D}][{AW}], unsigned sbase, unsigned tab)\n{{")
+    s.append("    asm volatile(")
+    s += e.lines
+    s.append("        : " + ", ".join(f'"+r"(acc[{j}][{i}])' for j in range(D) for i in range(AW)))
+    s.append('        : "r"(sbase), "r"(tab) : "memory");')
+    s.append("}\n")
+    s.append(f"template <> struct SlabU16PP<{D}, {T}, {NOFF}> {{ static constexpr int NCH = {NCH}; __device__ __forceinline__ static void run(unsigned (&a)[{D}][{AW}], unsigned sbase, unsigned tab) {{ {name}(a, sbase, tab); }} }};\n")
+    return "\n".join(s)
+
+
 # (D, T, NOFF) instances compiled into the library
 F32_VARIANTS = [(4, 28, 12), (4, 20, 12), (2, 28, 12)]
 U16_VARIANTS = [(4, 40, 16)]
 U16P_VARIANTS = [(2, 40, 12), (3, 40, 14)]
 F32P_VARIANTS = [(4, 28, 12), (4, 20, 12)]
+U16PP_VARIANTS = [(2, 40, 12)]
 
 
 def main(out):
@@ -448,6 +537,7 @@ def main(out):
     parts.append("template <int D, int T, int NOFF> struct SlabU16;   // packed u16x2 slab loop\n")
     parts.append("template <int D, int T, int NOFF> struct SlabU16P;  // two-phase packed u16x2 slab loop\n")
     parts.append("template <int D, int T, int NOFF> struct SlabF32P;  // packed f32x2 slab loop of the pair pre-sum mode\n")
+    parts.append("template <int D, int T, int NOFF> struct SlabU16PP; // two-phase packed u16x2 slab loop of the pair pre-sum mode\n")
     for v in F32_VARIANTS:
         parts.append(gen_f32(*v))
     for v in U16_VARIANTS:
@@ -456,6 +546,8 @@ def main(out):
         parts.append(gen_u16p(*v))
     for v in F32P_VARIANTS:
         parts.append(gen_f32p(*v))
+    for v in U16PP_VARIANTS:
+        parts.append(gen_u16pp(*v))
     txt = "\n".join(parts)
     if os.path.exists(out) and open(out).read() == txt:
         return

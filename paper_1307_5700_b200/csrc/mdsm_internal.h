@@ -40,7 +40,7 @@ struct TiledTables {
     int sigma_max = 0;
     // pair pre-sum mode (fp32): rows are (channel pair, delay difference) sums, see dedisperse_tiled.cu
     bool pairs = false;
-    int nslab_max = 0, nyrows = 0;                // slabs per block (padded), rows of the pre-summed copy per beam
+    int nslab_max = 0, nyrows = 0, nparts = 1;                // slabs per block (padded), rows of the pre-summed copy per beam
     int32_t *d_src_row = nullptr;                 // [n_dm_blocks][nslab_max*CS]  row of the pre-summed copy staged as row r (-1: none)
     int32_t *d_nslab_blk = nullptr;               // [n_dm_blocks]  slabs of this block
     int32_t *d_yrow_chan = nullptr, *d_yrow_delta = nullptr;   // [npairs + 1] first pre-summed row of every pair; [nyrows] delay difference of a row
@@ -70,6 +70,7 @@ struct mdsm_plan {
     int tiled_geom_f32 = -1, tiled_geom_u8 = -1;   // compiled tile geometry per dtype (option "tiled_geom_*"), -1 = automatic
     TiledTables tiled_f32, tiled_u8;
     void *d_pairs = nullptr; size_t pairs_bytes = 0;   // pre-summed channel pairs of an fp32 input (allocated on first use)
+    int pair_presum_u8 = 1;                            // option "pair_presum_u8" (integer kernel)
     int pair_presum = 1;                               // option "pair_presum" (fp32 only; falls back when the tables do not fit)
     void *d_widen = nullptr; size_t widen_bytes = 0;   // uint16 copy of a uint8 input (allocated on first use)
 

@@ -158,6 +158,11 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
         p->dedisp_kernel = (int)value;
         return MDSM_OK;
     }
+    if (strcmp(key, "pair_presum_u8") == 0) {
+        MDSM_REQUIRE(value == 0 || value == 1, "pair_presum_u8 must be 0 or 1");
+        p->pair_presum_u8 = (int)value;
+        return mdsm_tiled_build_tables(p);
+    }
     if (strcmp(key, "pair_presum") == 0) {
         MDSM_REQUIRE(value == 0 || value == 1, "pair_presum must be 0 or 1");
         p->pair_presum = (int)value;

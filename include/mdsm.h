@@ -62,7 +62,8 @@ const char *mdsm_last_error(void);
  * tile geometry, -1 (default) = the first one whose register window takes the plan's delay spread; if none does, or
  * rows are not 16-byte aligned, the direct kernel runs.  key "pair_presum" (default 1): fp32 dedispersion first sums
  * adjacent channel pairs for every delay difference the DM grid needs (exact, plan scratch of ~2 input sizes allocated
- * on the first call) and adds one window per pair; 0 = add every channel on its own.  keys "post_median_window" (0 = off, else odd <= 33) and
+ * on the first call) and adds one window per pair; 0 = add every channel on its own.  key "pair_presum_u8" (default
+ * 1): the same for uint8 input (uint16 pair sums, exact).  keys "post_median_window" (0 = off, else odd <= 33) and
  * "post_detrend" (0/1): mdsm_pipeline_host runs mdsm_median_filter / mdsm_detrend on the fp32 series between
  * dedispersion and detection (ignored for uint8 input).  Unknown key/value -> MDSM_EINVAL. */
 int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);

@@ -26,7 +26,7 @@ import numpy as np  # noqa: E402
 
 NOMINAL_ADD_PEAK = 148 * 128 * 1.965e9          # SMs x FP32/INT32 lanes x max SM clock (B200_PROFILING.md)
 # DRAM bytes of one dedispersion launch from the committed ncu captures (profiles/r1e_*.md); null for other configs
-NCU_TRAFFIC_BYTES = {"cfg3-8beam-f32": 17.8e9, "cfg4-8beam-u8": 2.44e9}
+NCU_TRAFFIC_BYTES = {"cfg3-8beam-f32": 17.8e9, "cfg4-8beam-u8": 6.73e9}
 
 
 def measured_hbm_peak() -> float:
@@ -342,7 +342,7 @@ def main():
                 "frac": adds / dd / peak, "peak_source": "measured in this run: mdsm_measure_add_peak (register-only add loop, all SMs)",
                 "peak_nominal": NOMINAL_ADD_PEAK / 1e9, "measured_peaks_gadd_s": {k: v / 1e9 for k, v in peaks.items()},
                 "ms_per_launch": dd * 1e3, "hbm_floor_ms": 1e3 * hbm_bytes / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full capture under profiles/ (r1i fp32: pre-pass 6.7 GB + tiled kernel 11.1 GB; r1h u8)"}
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full capture under profiles/ (r1i fp32: pre-pass 6.7 GB + tiled kernel 11.1 GB; r1k u8: pre-pass 2.77 GB + tiled kernel 3.96 GB)"}
 
     line = {
         "metric": "DM-trial samples/s", "value": value, "unit": "DM-trial samples/s", "n_gpus": world,

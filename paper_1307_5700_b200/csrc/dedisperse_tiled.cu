@@ -284,7 +284,7 @@ __global__ void __launch_bounds__((Tr::NW + Tr::PW) * 32, 1) dedisperse_tiled_ke
         const int b = a.beam0 + bb;
 #pragma unroll 1
         const int nslab_b = Tr::kPairs ? a.nslab_blk[blk] : a.nslab;
-        const int spp = Tr::kPairs ? nslab_b / a.nparts : a.slabs_per_part;
+        const int spp = !Tr::kPairs ? a.slabs_per_part : (Tr::kF32 ? nslab_b : nslab_b / a.nparts);   // fp32 tiles have one part
 #pragma unroll 1
         for (int s0 = 0; s0 < nslab_b; s0 += spp) {
 #pragma unroll

@@ -57,16 +57,28 @@ int64_t mdsm_plan_nsamps_out(const mdsm_plan *plan);                /* nsamps - 
 int mdsm_plan_get_delays(const mdsm_plan *plan, int32_t *h_delays);
 const char *mdsm_last_error(void);
 
-/* Plan options.  key "dedisp_kernel": 0 = auto, 1 = direct (global-load reference kernel),
- * 2 = tiled (shared-memory staged, register-blocked).  key "tiled_geom_f32" / "tiled_geom_u8": index of the compiled
- * tile geometry, -1 (default) = the first one whose register window takes the plan's delay spread; if none does, or
- * rows are not 16-byte aligned, the direct kernel runs.  key "pair_presum" (default 1): fp32 dedispersion first sums
- * adjacent channel pairs for every delay difference the DM grid needs (exact, plan scratch of ~2 input sizes allocated
- * on the first call) and adds one window per pair; 0 = add every channel on its own.  key "pair_presum_u8" (default
- * 1): the same for uint8 input (uint16 pair sums, exact).  keys "post_median_window" (0 = off, else odd <= 33) and
- * "post_detrend" (0/1): mdsm_pipeline_host runs mdsm_median_filter / mdsm_detrend on the fp32 series between
- * dedispersion and detection (ignored for uint8 input).  Unknown key/value -> MDSM_EINVAL. */
+/* Plan options (synchronise the device; not for use while work of this plan is in flight).
+ *  "dedisp_kernel": 0 = auto (the pre-summed-rows kernel whenever the plan has tables for it, else the direct kernel),
+ *      1 = direct (one thread per output, global loads: the cross-check kernel), 2 = pre-summed rows or MDSM_EINVAL.
+ *  "group_size": channels per pre-summed group, 1..8, or 0 (default) = the plan's cost model picks it.  Changing it
+ *      rebuilds the tables and DROPS the scratch reservation (call mdsm_plan_reserve again).
+ *  "post_median_window" (0 = off, else odd <= 33) and "post_detrend" (0/1): mdsm_pipeline_host runs
+ *      mdsm_median_filter / mdsm_detrend on the fp32 series between dedispersion and detection (ignored for uint8).
+ * Unknown key/value -> MDSM_EINVAL. */
 int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);
+/* Allocates the plan-owned scratch of mdsm_dedisperse for `dtype`: the exactly pre-summed channel-group rows
+ * (DESIGN.md section 6.1), nyrows * nsamps * (4 | 2) bytes per beam.  Call once after mdsm_plan_create (and after
+ * changing "group_size") and before the first mdsm_dedisperse of that dtype; mdsm_pipeline_host calls it itself.
+ * max_bytes = 0: as many beams as fit a quarter of the free device memory; otherwise at most max_bytes (never less
+ * than one beam).  When the scratch holds fewer beams than the plan (mdsm_plan_kernel_info: scratch_slots < nbeams),
+ * mdsm_dedisperse walks its beams through it in stream order and calls for different beam ranges must then be issued
+ * on ONE stream.  Synchronises the device only when an existing reservation has to be replaced.
+ * Returns MDSM_ENOMEM if not even one beam fits. */
+int mdsm_plan_reserve(mdsm_plan *plan, int dtype, int64_t max_bytes);
+/* Which dedispersion kernel mdsm_dedisperse runs for `dtype` and with what geometry: writes a NUL-terminated list of
+ * "key=value" words to buf ("kernel=rows group_size=4 ... scratch_slots=8 scratch_bytes=..." or
+ * "kernel=direct reason=option|no_tables").  Returns 1 (rows), 0 (direct) or a negative MDSM_* status. */
+int mdsm_plan_kernel_info(const mdsm_plan *plan, int dtype, char *buf, int64_t buflen);
 /* Number of kernels this plan has launched since creation (all entry points). */
 int64_t mdsm_plan_launch_count(const mdsm_plan *plan);
 

@@ -17,6 +17,7 @@ __all__ = [
     "EVENT_DTYPE", "MdsmError", "lib_path",
     "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
+    "mdsm_plan_reserve", "mdsm_plan_kernel_info",
     "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
 ]
 
@@ -60,6 +61,10 @@ def _load():
     L.mdsm_last_error.argtypes = []
     L.mdsm_plan_set_option.restype = c_int
     L.mdsm_plan_set_option.argtypes = [c_void_p, c_char_p, c_int64]
+    L.mdsm_plan_reserve.restype = c_int
+    L.mdsm_plan_reserve.argtypes = [c_void_p, c_int, c_int64]
+    L.mdsm_plan_kernel_info.restype = c_int
+    L.mdsm_plan_kernel_info.argtypes = [c_void_p, c_int, c_char_p, c_int64]
     L.mdsm_rfi_clip.restype = c_int
     L.mdsm_rfi_clip.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_double, c_double, c_void_p,
                                 c_void_p, c_void_p]
@@ -160,6 +165,26 @@ def mdsm_plan_get_delays(plan, ndms: int, nchans: int) -> np.ndarray:
 
 def mdsm_plan_set_option(plan, key: str, value: int) -> None:
     _check(_L.mdsm_plan_set_option(plan, key.encode(), value))
+
+
+def mdsm_plan_reserve(plan, dtype: int, max_bytes: int = 0) -> None:
+    _check(_L.mdsm_plan_reserve(plan, dtype, max_bytes))
+
+
+def mdsm_plan_kernel_info(plan, dtype: int) -> dict:
+    """The C call's "key=value ..." description as a dict (integers where they parse)."""
+    buf = ctypes.create_string_buffer(512)
+    rc = _L.mdsm_plan_kernel_info(plan, dtype, buf, len(buf))
+    if rc < 0:
+        raise MdsmError(rc, mdsm_last_error())
+    info = {}
+    for kv in buf.value.decode().split():
+        k, _, v = kv.partition("=")
+        try:
+            info[k] = int(v)
+        except ValueError:
+            info[k] = v
+    return info
 
 
 def mdsm_rfi_clip(plan, d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask=None, d_spec_mask=None,

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdsm.so")
-SOURCES = ["plan.cu", "clip.cu", "dedisperse_direct.cu", "dedisperse_tiled.cu", "detect.cu", "postprocess.cu", "power.cu", "mulaw.cu", "pipeline.cu", "add_peak.cu"]
+SOURCES = ["plan.cu", "clip.cu", "dedisperse_direct.cu", "dedisperse_rows.cu", "detect.cu", "postprocess.cu", "power.cu", "mulaw.cu", "pipeline.cu", "add_peak.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-O2,-ffp-contract=off", "-shared",
@@ -28,7 +28,6 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    subprocess.run([sys.executable, os.path.join(CSRC, "gen_chain.py"), os.path.join(CSRC, "chain_gen.h")], check=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, *NVCC_FLAGS, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:

@@ -1,0 +1,727 @@
+// Brute-force dedispersion for sm_100a as "exact channel-group pre-sums + a sum of shifted rows"
+// (BASELINE.json north_star item 2).
+//
+//   out[b][d][t] = sum_c in[b][c][t + delay(d,c)]
+//
+// Step 1, pre-pass (group_presum_*_kernel).  The channels are cut into groups of G adjacent channels
+// (c0 .. c0+G-1).  Inside a group the delays RELATIVE to its first channel,
+//   delta_i(d) = delay(d, c0+i) - delay(d, c0),   i = 1 .. G-1,
+// take only a few distinct values over the whole DM grid (cfg 3, G = 4: 5.7 patterns per channel on average),
+// because adjacent channels' delays differ by a few samples at most.  For every (group, pattern) the pre-pass
+// writes ONE row of plan scratch
+//   y[(g, pattern)][t] = sum_i in[c0+i][t + delta_i]
+// so that   out[d][t] = sum_g y[(g, pattern(d,g))][t + delay(d, c0_g)]:
+// exactly the same terms as the definition, added G at a time (uint8: bit-exact; fp32: another summation order,
+// inside the tolerance).  The main kernel then needs nchans/G adds and operand words per output instead of nchans.
+//
+// Step 2, main kernel (dedisperse_rows_kernel).  Persistent CTAs (one per SM) walk tiles = one beam x DB = NW*D
+// consecutive DM trials x `span` output samples.  A producer warp streams SLABS -- the y rows that the Q channel
+// groups of the slab need for this DM block, each row starting at its own 16-byte-aligned, delay-dependent sample --
+// into a ring of shared-memory stages with 1-D TMA bulk copies (cp.async.bulk ... mbarrier::complete_tx), together
+// with the slab's slice of the ENTRY table (one shared-memory byte offset per (DM, group)).  A consumer warp owns D DM
+// trials; lane l owns the outputs t0 + l + 32 i (i < T) of each of them (fp32) and adds, per (DM, group), the T words
+// at entry + 4 l + 128 i: conflict-free 32-bit shared-memory loads at ANY delay (no alignment cases, no register-offset
+// dispatch, no branches in the loop).  The kernel is bound by the shared-memory pipe at one operand word per add;
+// pre-summing is what makes a word worth G algorithmic adds.
+//   uint8: y holds uint16 group sums (G*255 < 2^16); a thread's accumulators are packed u16x2 lanes, one 32-bit
+//   shared-memory word = two samples.  A group whose offset is ODD relative to the word grid would need its words
+//   shifted by one lane; instead every DM keeps an even-phase row E (word k = outputs 2k, 2k+1) and an odd-phase row
+//   O (word k = outputs 2k-1, 2k) and both add the words as loaded; the rows are merged (one lane shuffle) when a
+//   PART of <= 256 channels (the most a 16-bit lane holds) is flushed into the uint32 output.
+// The time axis of a tile is SHEARED: DM dl of a block owns outputs [tile_t0 - sigma_dl, +span) with sigma_dl ~ half
+// the band-edge delay slope, which halves the length of the staged rows.
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <map>
+#include <vector>
+
+#include "mdsm_internal.h"
+
+namespace {
+
+// ------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{ .reg .b64 t; mbarrier.arrive.shared::cta.b64 t, [%0]; }" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("{ .reg .b64 t; mbarrier.arrive.expect_tx.shared::cta.b64 t, [%0], %1; }" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return done != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
+}
+// the producer runs several stages ahead, so it sleeps between polls instead of taking issue slots
+__device__ __forceinline__ void mbar_wait_sleep(uint64_t *bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) __nanosleep(200);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ------------------------------------------------------------------ step 1: the pre-pass
+constexpr int kGMax = 8;              // largest channel group
+constexpr int kPreThreads = 256;
+constexpr int kPreChunkF32 = 2048;    // samples of a y row per CTA (fp32): 8 per thread
+constexpr int kPreChunkU8 = 4096;     // uint8: 16 per thread, four at a time
+
+struct PreArgs {
+    const void *in;
+    void *y;
+    const int32_t *group_row0;        // [ngroups + 1] first y row of a group
+    const int16_t *ydelta;            // [nyrows][kGMax] delay of channel c0 + i relative to channel c0
+    int beam0, nslots, nchans, G, nyrows, dmax;
+    long long nsamps, ystride;
+};
+
+// fp32: one CTA = one channel group x one chunk of kPreChunkF32 samples x one beam.  The G raw rows of the chunk (plus
+// the largest delta) go to shared memory once and serve every pattern of the group; thread `tid` owns the samples
+// tid + 256 k, so that the shifted reads are conflict-free at any delta and the y stores are coalesced.
+template <int G>
+__global__ void __launch_bounds__(kPreThreads) group_presum_f32_kernel(const PreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *sm = reinterpret_cast<float *>(smem_raw);
+    const int g = blockIdx.y, b = a.beam0 + blockIdx.z;
+    const int c0 = g * a.G;
+    const long long t0 = (long long)blockIdx.x * kPreChunkF32;
+    const int pitch = kPreChunkF32 + a.dmax;
+    const float *in = reinterpret_cast<const float *>(a.in) + (size_t)b * a.nchans * (size_t)a.nsamps;
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const bool have = c0 + i < a.nchans;
+        const float *row = in + (size_t)(have ? c0 + i : 0) * a.nsamps;
+        for (int s = threadIdx.x; s < pitch; s += kPreThreads) sm[i * pitch + s] = (have && t0 + s < a.nsamps) ? row[t0 + s] : 0.0f;
+    }
+    __syncthreads();
+    const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    float *ybeam = reinterpret_cast<float *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
+    for (int r = row0; r < row1; ++r) {
+        int dl[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        float *yrow = ybeam + (size_t)r * a.ystride + t0;
+        float v[kPreChunkF32 / kPreThreads];
+#pragma unroll
+        for (int k = 0; k < kPreChunkF32 / kPreThreads; ++k) {
+            const int s = threadIdx.x + k * kPreThreads;
+            float acc = sm[s];                                   // delta_0 = 0
+#pragma unroll
+            for (int i = 1; i < G; ++i) acc += sm[i * pitch + s + dl[i]];
+            v[k] = acc;
+        }
+#pragma unroll
+        for (int k = 0; k < kPreChunkF32 / kPreThreads; ++k) {
+            const int s = threadIdx.x + k * kPreThreads;
+            if (t0 + s < a.ystride) yrow[s] = v[k];
+        }
+    }
+}
+
+// uint8 -> uint16 group sums.  Raw rows are kept as bytes; thread `tid` owns the samples 4 (tid + 256 k) .. +3: the four
+// bytes of row i at delta_i come out of two aligned words with one funnel shift (the shift is the same for the whole
+// row), are spread to two u16x2 words and added lane-wise; one 8-byte store per thread.
+template <int G>
+__global__ void __launch_bounds__(kPreThreads) group_presum_u8_kernel(const PreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int g = blockIdx.y, b = a.beam0 + blockIdx.z;
+    const int c0 = g * a.G;
+    const long long t0 = (long long)blockIdx.x * kPreChunkU8;
+    const int pitch = kPreChunkU8 + ((a.dmax + 3) & ~3) + 4;          // bytes, whole words, one spare word
+    const uint8_t *in = reinterpret_cast<const uint8_t *>(a.in) + (size_t)b * a.nchans * (size_t)a.nsamps;
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const bool have = c0 + i < a.nchans;
+        const uint8_t *row = in + (size_t)(have ? c0 + i : 0) * a.nsamps;
+        if ((((uintptr_t)(row + t0)) & 3) == 0) {
+            for (int s = threadIdx.x * 4; s < pitch; s += kPreThreads * 4) {
+                uint32_t w = 0;
+                if (have) {
+                    if (t0 + s + 3 < a.nsamps) w = *reinterpret_cast<const uint32_t *>(row + t0 + s);
+                    else
+                        for (int k = 0; k < 4; ++k)
+                            if (t0 + s + k < a.nsamps) w |= (uint32_t)row[t0 + s + k] << (8 * k);
+                }
+                *reinterpret_cast<uint32_t *>(smem_raw + i * pitch + s) = w;
+            }
+        } else {
+            for (int s = threadIdx.x; s < pitch; s += kPreThreads) smem_raw[i * pitch + s] = (have && t0 + s < a.nsamps) ? row[t0 + s] : (uint8_t)0;
+        }
+    }
+    __syncthreads();
+    const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    uint16_t *ybeam = reinterpret_cast<uint16_t *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
+    for (int r = row0; r < row1; ++r) {
+        int dl[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        uint16_t *yrow = ybeam + (size_t)r * a.ystride + t0;
+#pragma unroll
+        for (int k = 0; k < kPreChunkU8 / (4 * kPreThreads); ++k) {
+            const int s = 4 * (threadIdx.x + k * kPreThreads);
+            uint32_t lo = 0, hi = 0;
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const uint32_t *w = reinterpret_cast<const uint32_t *>(smem_raw + i * pitch + ((s + dl[i]) & ~3));
+                const uint32_t v = __funnelshift_r(w[0], w[1], 8 * (dl[i] & 3));
+                lo += __byte_perm(v, 0, 0x4140);
+                hi += __byte_perm(v, 0, 0x4342);
+            }
+            if (t0 + s < a.ystride) *reinterpret_cast<uint2 *>(yrow + s) = make_uint2(lo, hi);      // ystride % 8 == 0
+        }
+    }
+}
+
+// ------------------------------------------------------------------ step 2: the sum of shifted rows
+struct RowsArgs {
+    const void *y;                    // [nslots][nyrows][ystride] pre-summed rows
+    void *out;
+    const int4 *rowdesc;              // [nblk][nslab][CS]: (y row or -1, first staged sample - tile_t0, samples to copy, 0)
+    const uint32_t *ent;              // [nblk][nslab][DB*Q] byte offset of the (DM, group) window inside a stage (uint16: | odd)
+    const int32_t *sigma;             // [DB] output time shear per DM of a block
+    int beam0, nslots, nyrows, ndms;
+    int nblk, ntile_t, nslab, Q, ngroups, CS, pitch, stages, slabs_per_part;
+    int stride;                       // outputs a tile owns per DM (its time step)
+    long long ntiles, nsamps, nsamps_out, ystride;
+};
+
+template <int D_, int T_, int NW_, bool F32_> struct RowsTraits {
+    static constexpr int D = D_, T = T_, NW = NW_;
+    static constexpr bool kF32 = F32_;
+    static constexpr int kSpan = F32_ ? 32 * T_ : 64 * T_;          // samples a warp's accumulators cover per DM
+    using Y = typename std::conditional<F32_, float, uint16_t>::type;
+};
+
+template <typename Tr>
+__global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(const RowsArgs a)
+{
+    using Y = typename Tr::Y;
+    constexpr int D = Tr::D, T = Tr::T, NW = Tr::NW, DB = D * NW;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int stages = a.stages;
+    const uint32_t row_bytes = (uint32_t)a.pitch * sizeof(Y);
+    const uint32_t ent_bytes = (uint32_t)(DB * a.Q) * 4u;
+    const uint32_t stage_bytes = (a.CS * row_bytes + ent_bytes + 127u) & ~127u;     // rows, then the entry slice
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)stages * stage_bytes);
+    uint64_t *empty = full + stages;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // Rows that stick out of [0, ystride) are only partly written by the bulk copies.  What they leave behind feeds
+    // outputs outside [0, nsamps_out) only, but a stale 16-bit lane must never carry into its valid neighbour: with
+    // the stages zeroed once, every staged value is zero or a real group sum.
+    for (uint32_t i = threadIdx.x; i < stages * stage_bytes / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[s], 32);
+            mbar_init(&empty[s], NW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == NW) {
+        // ===== producer: lane r copies row r of every slab, lane 0 also the slab's slice of the entry table =====
+        int st = 0;
+        uint32_t ph = 1;             // parity of the empty-barrier phase to wait for (first lap: no wait)
+        bool first_lap = true;
+        const uint32_t smem0 = smem_u32(smem);
+        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+            const int blk = (int)(tile % a.nblk);
+            const long long rest = tile / a.nblk;
+            const int tt = (int)(rest % a.ntile_t), bb = (int)(rest / a.ntile_t);
+            const long long tile_t0 = (long long)tt * a.stride;
+            const Y *ybeam = reinterpret_cast<const Y *>(a.y) + (size_t)((a.beam0 + bb) % a.nslots) * a.nyrows * (size_t)a.ystride;
+            const int4 *rd = a.rowdesc + (size_t)blk * a.nslab * a.CS;
+            const uint32_t *et = a.ent + (size_t)blk * a.nslab * (DB * a.Q);
+            int4 desc = lane < a.CS ? rd[lane] : make_int4(-1, 0, 0, 0);
+            for (int slab = 0; slab < a.nslab; ++slab) {
+                const int4 cur = desc;
+                if (slab + 1 < a.nslab && lane < a.CS) desc = rd[(size_t)(slab + 1) * a.CS + lane];     // next slab's rows, before the wait
+                if (!first_lap) mbar_wait_sleep(&empty[st], ph);
+                const uint32_t sbase = smem0 + st * stage_bytes;
+                uint32_t bytes = 0;
+                long long lo = 0, g0 = 0;
+                if (cur.x >= 0) {
+                    g0 = tile_t0 + cur.y;
+                    lo = g0 < 0 ? 0 : g0;
+                    long long hi = g0 + cur.z;
+                    if (hi > a.ystride) hi = a.ystride;
+                    if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(Y));
+                }
+                mbar_arrive_expect_tx(&full[st], bytes + (lane == 0 ? ent_bytes : 0u));
+                if (bytes) bulk_g2s(sbase + lane * row_bytes + (uint32_t)((lo - g0) * sizeof(Y)), ybeam + (size_t)cur.x * a.ystride + lo, bytes, &full[st]);
+                if (lane == 0) bulk_g2s(sbase + a.CS * row_bytes, et + (size_t)slab * (DB * a.Q), ent_bytes, &full[st]);
+                if (++st == stages) { st = 0; ph ^= 1; first_lap = false; }
+            }
+        }
+        return;
+    }
+
+    // ===== consumer warps =====
+    const int Q = a.Q;
+    int st = 0;
+    uint32_t ph = 0;
+    for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+        const int blk = (int)(tile % a.nblk);
+        const long long rest = tile / a.nblk;
+        const int tt = (int)(rest % a.ntile_t), bb = (int)(rest / a.ntile_t);
+        const long long tile_t0 = (long long)tt * a.stride;
+        const int b = a.beam0 + bb;
+        if constexpr (Tr::kF32) {
+            float acc[D][T];
+#pragma unroll
+            for (int j = 0; j < D; ++j)
+#pragma unroll
+                for (int i = 0; i < T; ++i) acc[j][i] = 0.0f;
+#pragma unroll 1
+            for (int slab = 0; slab < a.nslab; ++slab) {
+                const int nq = min(Q, a.ngroups - slab * Q);
+                mbar_wait(&full[st], ph);
+                const unsigned char *sbase = smem + (size_t)st * stage_bytes;
+                const uint32_t *ents = reinterpret_cast<const uint32_t *>(sbase + a.CS * row_bytes) + warp * D * Q;
+#pragma unroll 1
+                for (int q = 0; q < nq; ++q) {
+                    uint32_t e[D];
+#pragma unroll
+                    for (int j = 0; j < D; ++j) e[j] = ents[j * Q + q];
+#pragma unroll
+                    for (int j = 0; j < D; ++j) {
+                        const float *w = reinterpret_cast<const float *>(sbase + e[j]) + lane;
+                        float v[T];
+#pragma unroll
+                        for (int i = 0; i < T; ++i) v[i] = w[32 * i];
+#pragma unroll
+                        for (int i = 0; i < T; ++i) acc[j][i] += v[i];
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
+                if (++st == stages) { st = 0; ph ^= 1; }
+            }
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const int dl = warp * D + j, d = blk * DB + dl;
+                if (d >= a.ndms) continue;
+                const int sg = a.sigma[dl];
+                float *orow = reinterpret_cast<float *>(a.out) + ((size_t)b * a.ndms + d) * (size_t)a.nsamps;
+#pragma unroll
+                for (int i = 0; i < T; ++i) {
+                    const long long t = tile_t0 - sg + lane + 32 * i;
+                    if (t >= 0 && t < a.nsamps_out) orow[t] = acc[j][i];
+                }
+            }
+        } else {
+            uint32_t accE[D][T], accO[D][T];
+#pragma unroll 1
+            for (int s0 = 0; s0 < a.nslab; s0 += a.slabs_per_part) {
+#pragma unroll
+                for (int j = 0; j < D; ++j)
+#pragma unroll
+                    for (int i = 0; i < T; ++i) { accE[j][i] = 0; accO[j][i] = 0; }
+                const int s1 = min(a.nslab, s0 + a.slabs_per_part);
+#pragma unroll 1
+                for (int slab = s0; slab < s1; ++slab) {
+                    const int nq = min(Q, a.ngroups - slab * Q);
+                    mbar_wait(&full[st], ph);
+                    const unsigned char *sbase = smem + (size_t)st * stage_bytes;
+                    const uint32_t *ents = reinterpret_cast<const uint32_t *>(sbase + a.CS * row_bytes) + warp * D * Q;
+#pragma unroll 1
+                    for (int q = 0; q < nq; ++q) {
+                        uint32_t e[D];
+#pragma unroll
+                        for (int j = 0; j < D; ++j) e[j] = ents[j * Q + q];
+#pragma unroll
+                        for (int j = 0; j < D; ++j) {
+                            const uint32_t *w = reinterpret_cast<const uint32_t *>(sbase + (e[j] & ~3u)) + lane;
+                            uint32_t v[T];
+#pragma unroll
+                            for (int i = 0; i < T; ++i) v[i] = w[32 * i];
+                            if (e[j] & 1u) {
+#pragma unroll
+                                for (int i = 0; i < T; ++i) accO[j][i] += v[i];
+                            } else {
+#pragma unroll
+                                for (int i = 0; i < T; ++i) accE[j][i] += v[i];
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[st]);
+                    if (++st == stages) { st = 0; ph ^= 1; }
+                }
+                // ----- flush of the part: out(2k) = E_k.lo + O_k.hi, out(2k+1) = E_k.hi + O_{k+1}.lo, word k = lane + 32 i -----
+#pragma unroll
+                for (int j = 0; j < D; ++j) {
+                    const int dl = warp * D + j, d = blk * DB + dl;
+                    const long long ts = tile_t0 - a.sigma[dl] + 2 * lane;
+                    uint32_t *orow = reinterpret_cast<uint32_t *>(a.out) + ((size_t)b * a.ndms + (d < a.ndms ? d : 0)) * (size_t)a.nsamps;
+                    uint32_t v0[T], v1[T];
+                    bool ok0[T], ok1[T];
+#pragma unroll
+                    for (int i = 0; i < T; ++i) {
+                        const uint32_t up = __shfl_sync(0xffffffffu, accO[j][i], (lane + 1) & 31);
+                        const uint32_t wrap = __shfl_sync(0xffffffffu, accO[j][i + 1 < T ? i + 1 : i], 0);
+                        const uint32_t onext = lane == 31 ? wrap : up;
+                        v0[i] = (accE[j][i] & 0xffffu) + (accO[j][i] >> 16);
+                        v1[i] = (accE[j][i] >> 16) + (onext & 0xffffu);
+                        const int k2 = 2 * (lane + 32 * i);
+                        const long long t = ts + 64 * i;
+                        ok0[i] = d < a.ndms && k2 < a.stride && t >= 0 && t < a.nsamps_out;
+                        ok1[i] = d < a.ndms && k2 + 1 < a.stride && t + 1 >= 0 && t + 1 < a.nsamps_out;
+                    }
+                    if (s0 != 0) {
+                        // later parts add to what part 0 stored: this thread's own elements (still in L2); all the loads
+                        // are issued before the first store so that their latencies overlap
+                        uint32_t o0[T], o1[T];
+#pragma unroll
+                        for (int i = 0; i < T; ++i) {
+                            o0[i] = ok0[i] ? __ldcg(orow + ts + 64 * i) : 0u;
+                            o1[i] = ok1[i] ? __ldcg(orow + ts + 64 * i + 1) : 0u;
+                        }
+#pragma unroll
+                        for (int i = 0; i < T; ++i) { v0[i] += o0[i]; v1[i] += o1[i]; }
+                    }
+#pragma unroll
+                    for (int i = 0; i < T; ++i) {
+                        if (ok0[i]) orow[ts + 64 * i] = v0[i];
+                        if (ok1[i]) orow[ts + 64 * i + 1] = v1[i];
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------ host side: the plan-time tables
+struct RowsGeom { int D, T, NW; };
+constexpr RowsGeom kGeomRowsF32 = {4, 16, 16};      // 64 DMs x 512 samples per tile
+constexpr RowsGeom kGeomRowsU16 = {4, 8, 16};       // 64 DMs x 512 samples (504 owned) per tile
+constexpr int kPartChans = 256;                     // 256 * 255 < 2^16: the most channels a 16-bit lane can take
+constexpr size_t kSmemBudget = 227 * 1024;
+
+static inline long long floor_to(long long v, int a) { return v >= 0 ? (v / a) * a : -(((-v) + a - 1) / a) * a; }
+static inline long long ceil_to(long long v, int a) { return -floor_to(-v, a); }
+
+template <typename V> static bool upload(V **dptr, const std::vector<V> &h)
+{
+    if (cudaMalloc((void **)dptr, std::max<size_t>(h.size(), 1) * sizeof(V)) != cudaSuccess) return false;
+    return h.empty() || cudaMemcpy(*dptr, h.data(), h.size() * sizeof(V), cudaMemcpyHostToDevice) == cudaSuccess;
+}
+
+// y rows of a group size: every pattern of relative delays a group takes over the DM grid
+struct GroupRows {
+    int G = 0, ngroups = 0, nyrows = 0, dmax = 0;
+    std::vector<int32_t> yrow_of;          // [ndms][ngroups]
+    std::vector<int32_t> group_row0;       // [ngroups + 1]
+    std::vector<int16_t> ydelta;           // [nyrows][kGMax]
+};
+
+static bool enumerate_group_rows(const mdsm_plan *p, int G, GroupRows &gr)
+{
+    gr.G = G;
+    gr.ngroups = (p->nchans + G - 1) / G;
+    gr.yrow_of.assign((size_t)p->ndms * gr.ngroups, 0);
+    gr.group_row0.assign(gr.ngroups + 1, 0);
+    gr.ydelta.clear();
+    gr.dmax = 0;
+    int nrows = 0;
+    for (int g = 0; g < gr.ngroups; ++g) {
+        gr.group_row0[g] = nrows;
+        std::map<std::array<int16_t, kGMax>, int> seen;
+        const int c0 = g * G;
+        std::array<int16_t, kGMax> last{};
+        int last_row = -1;
+        for (int d = 0; d < p->ndms; ++d) {
+            const int32_t *row = p->h_delay.data() + (size_t)d * p->nchans;
+            std::array<int16_t, kGMax> pat{};
+            for (int i = 1; i < G && c0 + i < p->nchans; ++i) {
+                const long long de = (long long)row[c0 + i] - row[c0];
+                if (de < 0 || de > 4000) return false;          // not a dispersion sweep this scheme is meant for
+                pat[i] = (int16_t)de;
+                gr.dmax = std::max(gr.dmax, (int)de);
+            }
+            if (d > 0 && pat == last) {                         // neighbouring DMs mostly share the pattern
+                gr.yrow_of[(size_t)d * gr.ngroups + g] = last_row;
+                continue;
+            }
+            auto it = seen.find(pat);
+            if (it == seen.end()) {
+                it = seen.emplace(pat, nrows++).first;
+                gr.ydelta.insert(gr.ydelta.end(), pat.begin(), pat.end());
+            }
+            gr.yrow_of[(size_t)d * gr.ngroups + g] = it->second;
+            last = pat;
+            last_row = it->second;
+        }
+    }
+    gr.group_row0[gr.ngroups] = nrows;
+    gr.nyrows = nrows;
+    return true;
+}
+
+struct RowsHost {
+    std::vector<int4> rowdesc;
+    std::vector<uint32_t> ent;
+    std::vector<int32_t> sigma;
+};
+
+// Builds the per-block staging lists and entry tables for one dtype, group size and geometry.
+static bool build_rows_tables(const mdsm_plan *p, bool f32, const GroupRows &gr, const RowsGeom &g, RowsTables &rt, RowsHost &h)
+{
+    const int al = f32 ? 4 : 8, esize = f32 ? 4 : 2;
+    const int DB = g.D * g.NW;
+    const int span = f32 ? 32 * g.T : 64 * g.T;
+    const int stride = f32 ? span : span - 8;
+    const int nblk = (p->ndms + DB - 1) / DB;
+    const int ng = gr.ngroups, G = gr.G;
+    // un-rounded delay increment per DM step at the band edge: the slope the shear splits in half
+    const double f_lo = p->f_top + (p->nchans - 1) * p->foff;
+    const double smax = 4.148808e3 * p->dm_step * (1.0 / (f_lo * f_lo) - 1.0 / (p->f_top * p->f_top)) / p->tsamp;
+    h.sigma.resize(DB);
+    for (int dl = 0; dl < DB; ++dl) h.sigma[dl] = (int32_t)llround(0.5 * smax * dl);
+    auto dly = [&](int d, int c) { return (long long)p->h_delay[(size_t)d * p->nchans + c]; };
+
+    // per block and group: the distinct y rows its DMs use, with the range of window starts
+    struct Use { int yrow; long long emin, emax; };
+    std::vector<std::vector<Use>> uses((size_t)nblk * ng);
+    long long need_max = 0;
+    for (int blk = 0; blk < nblk; ++blk)
+        for (int gi = 0; gi < ng; ++gi) {
+            auto &u = uses[(size_t)blk * ng + gi];
+            for (int dl = 0; dl < DB; ++dl) {
+                const int d = blk * DB + dl;
+                if (d >= p->ndms) break;
+                const int yr = gr.yrow_of[(size_t)d * ng + gi];
+                const long long e = dly(d, gi * G) - h.sigma[dl];
+                auto it = std::find_if(u.begin(), u.end(), [&](const Use &x) { return x.yrow == yr; });
+                if (it == u.end()) u.push_back({yr, e, e});
+                else { it->emin = std::min(it->emin, e); it->emax = std::max(it->emax, e); }
+            }
+            for (const Use &x : u) need_max = std::max(need_max, x.emax - floor_to(x.emin, al) + span);
+        }
+    const int pitch = (int)ceil_to(need_max, al);
+    // groups per slab: as many as keep a slab within 32 rows (one per producer lane) and three stages in shared memory
+    const int part_groups_max = f32 ? ng : std::max(1, kPartChans / G);
+    int Q = 0, CS = 0;
+    for (int q : {4, 3, 2, 1}) {
+        if (!f32 && part_groups_max % q) continue;
+        if ((DB * q) % 4) continue;
+        int cs = 0;
+        for (int blk = 0; blk < nblk; ++blk)
+            for (int s0 = 0; s0 < ng; s0 += q) {
+                int n = 0;
+                for (int gi = s0; gi < std::min(ng, s0 + q); ++gi) n += (int)uses[(size_t)blk * ng + gi].size();
+                cs = std::max(cs, n);
+            }
+        const size_t stage = (((size_t)cs * pitch * esize + (size_t)DB * q * 4) + 127) & ~(size_t)127;
+        if (cs <= 32 && 3 * stage + 256 <= kSmemBudget) { Q = q; CS = cs; break; }
+    }
+    if (!Q) return false;
+    const int nslab = (ng + Q - 1) / Q;
+    h.rowdesc.assign((size_t)nblk * nslab * CS, make_int4(-1, 0, 0, 0));
+    h.ent.assign((size_t)nblk * nslab * DB * Q, 0u);
+    for (int blk = 0; blk < nblk; ++blk)
+        for (int slab = 0; slab < nslab; ++slab) {
+            int r = 0;
+            for (int q = 0; q < Q; ++q) {
+                const int gi = slab * Q + q;
+                if (gi >= ng) break;
+                const auto &u = uses[(size_t)blk * ng + gi];
+                for (size_t k = 0; k < u.size(); ++k) {
+                    const long long rs = floor_to(u[k].emin, al);
+                    const long long len = ceil_to(u[k].emax - rs + span, al);
+                    h.rowdesc[((size_t)blk * nslab + slab) * CS + r + k] = make_int4(u[k].yrow, (int)rs, (int)len, 0);
+                }
+                for (int dl = 0; dl < DB; ++dl) {
+                    const int d = std::min(blk * DB + dl, p->ndms - 1);
+                    const int dle = d - blk * DB;                           // a DM past the grid repeats the last one (never stored)
+                    const int yr = gr.yrow_of[(size_t)d * ng + gi];
+                    size_t k = 0;
+                    while (u[k].yrow != yr) ++k;
+                    const long long o = dly(d, gi * G) - h.sigma[dle] - floor_to(u[k].emin, al);
+                    uint32_t e;
+                    if (f32) e = (uint32_t)(((long long)(r + k) * pitch + o) * 4);
+                    else e = (uint32_t)(((long long)(r + k) * pitch + (o & ~1LL)) * 2) | (uint32_t)(o & 1);
+                    h.ent[(((size_t)blk * nslab + slab) * DB + dl) * Q + q] = e;
+                }
+                r += (int)u.size();
+            }
+        }
+    rt.G = G; rt.D = g.D; rt.T = g.T; rt.NW = g.NW; rt.DB = DB; rt.span = span; rt.stride = stride;
+    rt.Q = Q; rt.CS = CS; rt.pitch = pitch; rt.nslab = nslab; rt.nblk = nblk; rt.ngroups = ng; rt.nyrows = gr.nyrows;
+    rt.dmax = gr.dmax;
+    rt.slabs_per_part = f32 ? nslab : part_groups_max / Q;
+    rt.ystride = ceil_to(p->nsamps, al);
+    rt.sigma_max = *std::max_element(h.sigma.begin(), h.sigma.end());
+    const size_t stage = (((size_t)CS * pitch * esize + (size_t)DB * Q * 4) + 127) & ~(size_t)127;
+    rt.stages = (int)std::min<size_t>(8, (kSmemBudget - 256) / stage);
+    rt.smem_bytes = (size_t)rt.stages * stage + 2 * rt.stages * sizeof(uint64_t);
+    long long rows_staged = 0;
+    for (const auto &u : uses) rows_staged += (long long)u.size();
+    rt.rows_per_block = (double)rows_staged / nblk;
+    return true;
+}
+
+static void free_rows_tables(RowsTables *rt)
+{
+    cudaFree(rt->d_rowdesc); cudaFree(rt->d_ent); cudaFree(rt->d_sigma); cudaFree(rt->d_group_row0); cudaFree(rt->d_ydelta);
+    *rt = RowsTables();
+}
+
+// Modelled cost of a group size in units of one shared-memory operand word per output sample: nchans/G words in the
+// main kernel, plus the y rows, each written to and read back from HBM (about 14 word-times per row and sample).
+static double group_cost(const mdsm_plan *p, const GroupRows &gr) { return (double)p->ndms * gr.ngroups + 14.0 * gr.nyrows; }
+
+static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &cands)
+{
+    RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
+    free_rows_tables(&rt);
+    const RowsGeom geom = f32 ? kGeomRowsF32 : kGeomRowsU16;
+    // candidates in the order of their modelled cost; the first whose tables fit the kernel's limits is taken
+    std::vector<const GroupRows *> order;
+    for (const GroupRows &gr : cands) order.push_back(&gr);
+    std::sort(order.begin(), order.end(), [&](const GroupRows *x, const GroupRows *y) { return group_cost(p, *x) < group_cost(p, *y); });
+    for (const GroupRows *gr : order) {
+        RowsHost h;
+        if (!build_rows_tables(p, f32, *gr, geom, rt, h)) continue;
+        if (!upload((int4 **)&rt.d_rowdesc, h.rowdesc) || !upload(&rt.d_ent, h.ent) || !upload(&rt.d_sigma, h.sigma) ||
+            !upload(&rt.d_group_row0, gr->group_row0) || !upload(&rt.d_ydelta, gr->ydelta)) {
+            mdsm_set_error("dedispersion table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+            free_rows_tables(&rt);
+            return MDSM_ECUDA;
+        }
+        rt.ok = true;
+        return MDSM_OK;
+    }
+    return MDSM_OK;                                                    // no table: the direct kernel runs
+}
+
+template <int G> static void launch_presum(bool f32, const PreArgs &a, dim3 grid, size_t smem, cudaStream_t st)
+{
+    if (f32) group_presum_f32_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
+    else group_presum_u8_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
+}
+
+template <typename Tr> static int launch_rows(const RowsArgs &a, size_t smem, int grid, cudaStream_t st)
+{
+    auto kern = dedisperse_rows_kernel<Tr>;
+    // per launch: the attribute belongs to the current device's copy of the kernel, and the call costs microseconds
+    MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, (Tr::NW + 1) * 32, smem, st>>>(a);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    return MDSM_OK;
+}
+
+}  // namespace
+
+int mdsm_rows_build_tables(mdsm_plan *p)
+{
+    std::vector<GroupRows> cands;
+    for (int G = 1; G <= kGMax; ++G) {
+        if (p->group_size > 0 && G != p->group_size) continue;
+        GroupRows gr;
+        if (enumerate_group_rows(p, G, gr)) cands.push_back(std::move(gr));
+    }
+    int rc = build_dtype(p, true, cands);
+    if (rc == MDSM_OK) rc = build_dtype(p, false, cands);
+    return rc;
+}
+
+void mdsm_rows_free_tables(mdsm_plan *p)
+{
+    free_rows_tables(&p->rows_f32);
+    free_rows_tables(&p->rows_u8);
+}
+
+size_t mdsm_rows_scratch_bytes_per_beam(const mdsm_plan *p, int dtype)
+{
+    const RowsTables &rt = dtype == MDSM_F32 ? p->rows_f32 : p->rows_u8;
+    return rt.ok ? (size_t)rt.nyrows * (size_t)rt.ystride * (dtype == MDSM_F32 ? 4 : 2) : 0;
+}
+
+int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out, cudaStream_t st)
+{
+    const bool f32 = dtype == MDSM_F32;
+    const RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
+    void *scratch = f32 ? p->d_scratch_f32 : p->d_scratch_u8;
+    const int nslots = f32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
+    MDSM_REQUIRE(rt.ok && scratch && nslots >= 1, "dedispersion scratch not reserved (call mdsm_plan_reserve)");
+    const int ntile_t = (int)((p->nsamps_out + rt.sigma_max + rt.stride - 1) / rt.stride);
+    const int chunk = f32 ? kPreChunkF32 : kPreChunkU8;
+    const size_t pre_smem = f32 ? (size_t)rt.G * (chunk + rt.dmax) * sizeof(float) : (size_t)rt.G * (chunk + ((rt.dmax + 3) & ~3) + 4);
+    MDSM_REQUIRE(pre_smem <= 200 * 1024, "pre-pass: group delay range too large");
+    // beams go through the scratch `nslots` at a time (slot = beam % nslots), in stream order
+    for (int bs = beam0; bs < beam0 + nb; bs += nslots) {
+        const int n = std::min(nslots, beam0 + nb - bs);
+        PreArgs pa;
+        pa.in = d_in; pa.y = scratch; pa.group_row0 = rt.d_group_row0; pa.ydelta = rt.d_ydelta;
+        pa.beam0 = bs; pa.nslots = nslots; pa.nchans = p->nchans; pa.G = rt.G; pa.nyrows = rt.nyrows; pa.dmax = rt.dmax;
+        pa.nsamps = p->nsamps; pa.ystride = rt.ystride;
+        dim3 grid((unsigned)((rt.ystride + chunk - 1) / chunk), rt.ngroups, n);
+        MDSM_REQUIRE(rt.ngroups <= 65535 && n <= 65535, "pre-pass: grid too large");
+        if (pre_smem > 48 * 1024) {
+            // only very wide groups need this; set per launch (per-device state)
+            switch (rt.G) {
+#define MDSM_PRE_ATTR(GG) case GG: \
+                MDSM_CUDA_TRY(cudaFuncSetAttribute(group_presum_f32_kernel<GG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pre_smem)); \
+                MDSM_CUDA_TRY(cudaFuncSetAttribute(group_presum_u8_kernel<GG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pre_smem)); break;
+                MDSM_PRE_ATTR(1) MDSM_PRE_ATTR(2) MDSM_PRE_ATTR(3) MDSM_PRE_ATTR(4) MDSM_PRE_ATTR(5) MDSM_PRE_ATTR(6) MDSM_PRE_ATTR(7) MDSM_PRE_ATTR(8)
+#undef MDSM_PRE_ATTR
+            }
+        }
+        switch (rt.G) {
+            case 1: launch_presum<1>(f32, pa, grid, pre_smem, st); break;
+            case 2: launch_presum<2>(f32, pa, grid, pre_smem, st); break;
+            case 3: launch_presum<3>(f32, pa, grid, pre_smem, st); break;
+            case 4: launch_presum<4>(f32, pa, grid, pre_smem, st); break;
+            case 5: launch_presum<5>(f32, pa, grid, pre_smem, st); break;
+            case 6: launch_presum<6>(f32, pa, grid, pre_smem, st); break;
+            case 7: launch_presum<7>(f32, pa, grid, pre_smem, st); break;
+            default: launch_presum<8>(f32, pa, grid, pre_smem, st); break;
+        }
+        MDSM_CUDA_TRY(cudaGetLastError());
+        p->launches += 1;
+
+        RowsArgs a;
+        a.y = scratch; a.out = d_out;
+        a.rowdesc = (const int4 *)rt.d_rowdesc; a.ent = rt.d_ent; a.sigma = rt.d_sigma;
+        a.beam0 = bs; a.nslots = nslots; a.nyrows = rt.nyrows; a.ndms = p->ndms;
+        a.nblk = rt.nblk; a.ntile_t = ntile_t; a.nslab = rt.nslab; a.Q = rt.Q; a.ngroups = rt.ngroups; a.CS = rt.CS;
+        a.pitch = rt.pitch; a.stages = rt.stages; a.slabs_per_part = rt.slabs_per_part; a.stride = rt.stride;
+        a.ntiles = (long long)rt.nblk * ntile_t * n;
+        a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out; a.ystride = rt.ystride;
+        const int grid_main = (int)std::min<long long>(a.ntiles, p->sm_count);
+        int rc;
+        if (f32) rc = launch_rows<RowsTraits<kGeomRowsF32.D, kGeomRowsF32.T, kGeomRowsF32.NW, true>>(a, rt.smem_bytes, grid_main, st);
+        else rc = launch_rows<RowsTraits<kGeomRowsU16.D, kGeomRowsU16.T, kGeomRowsU16.NW, false>>(a, rt.smem_bytes, grid_main, st);
+        if (rc != MDSM_OK) return rc;
+        p->launches += 1;
+    }
+    return MDSM_OK;
+}

@@ -27,25 +27,23 @@ void mdsm_set_error(const char *fmt, ...);
         }                                \
     } while (0)
 
-// Geometry of the tiled dedispersion kernel (see dedisperse_tiled.cu and DESIGN.md section 6).
-struct TiledTables {
-    int dms_per_warp = 0, warps = 0, tpt = 0, cs = 0;   // D, NW, T (samples per thread), channels per slab
-    int dm_block = 0, n_dm_blocks = 0;            // DB = D*NW
-    int tile_t = 0;                               // 32*T output samples per CTA
-    int row_words = 0;                            // staged elements (f32 / u16) per channel row
-    int max_off = 0;                              // largest per-DM register offset
-    int32_t *d_row_start = nullptr;               // [n_dm_blocks][nchans]   first staged sample - tile_t0
-    void *d_warp_tab = nullptr;                   // [n_dm_blocks][nslab][warps][CS] packed window base + per-DM offsets
-    int32_t *d_sigma = nullptr;                   // [n_dm_blocks*dm_block]  output time shear per DM
-    int sigma_max = 0;
-    // pair pre-sum mode (fp32): rows are (channel pair, delay difference) sums, see dedisperse_tiled.cu
-    bool pairs = false;
-    int nslab_max = 0, nyrows = 0, nparts = 1;                // slabs per block (padded), rows of the pre-summed copy per beam
-    int32_t *d_src_row = nullptr;                 // [n_dm_blocks][nslab_max*CS]  row of the pre-summed copy staged as row r (-1: none)
-    int32_t *d_nslab_blk = nullptr;               // [n_dm_blocks]  slabs of this block
-    int32_t *d_yrow_chan = nullptr, *d_yrow_delta = nullptr;   // [npairs + 1] first pre-summed row of every pair; [nyrows] delay difference of a row
-    int geom = 0;                                 // index of the compiled geometry the tables were built for
+// Plan-time tables of the dedispersion kernels (see dedisperse_rows.cu and DESIGN.md section 6.1).
+struct RowsTables {
     bool ok = false;
+    int G = 0;                                    // channels per pre-summed group
+    int D = 0, T = 0, NW = 0, DB = 0;             // DMs per warp, words per thread and DM, consumer warps, DMs per block
+    int span = 0, stride = 0;                     // samples a tile's accumulators cover per DM / outputs it owns (its time step)
+    int Q = 0, CS = 0, pitch = 0;                 // groups per slab, row slots per stage, elements per row slot
+    int nslab = 0, nblk = 0, ngroups = 0, nyrows = 0, dmax = 0, slabs_per_part = 0;
+    long long ystride = 0;                        // elements per y row (nsamps rounded up to 16 bytes)
+    int sigma_max = 0, stages = 0;
+    size_t smem_bytes = 0;
+    double rows_per_block = 0.0;                  // y rows a DM block stages per tile (statistics for kernel_info)
+    void *d_rowdesc = nullptr;                    // int4 [nblk][nslab][CS]
+    uint32_t *d_ent = nullptr;                    // [nblk][nslab][DB*Q]
+    int32_t *d_sigma = nullptr;                   // [DB]
+    int32_t *d_group_row0 = nullptr;              // [ngroups + 1]
+    int16_t *d_ydelta = nullptr;                  // [nyrows][8]
 };
 
 struct mdsm_plan {
@@ -66,13 +64,12 @@ struct mdsm_plan {
     // detect scratch
     double *d_series_stats = nullptr; // [nbeams][ndms][2] = mean, rms
 
-    int dedisp_kernel = 0;            // 0 auto, 1 direct, 2 tiled
-    int tiled_geom_f32 = -1, tiled_geom_u8 = -1;   // compiled tile geometry per dtype (option "tiled_geom_*"), -1 = automatic
-    TiledTables tiled_f32, tiled_u8;
-    void *d_pairs = nullptr; size_t pairs_bytes = 0;   // pre-summed channel pairs of an fp32 input (allocated on first use)
-    int pair_presum_u8 = 1;                            // option "pair_presum_u8" (integer kernel)
-    int pair_presum = 1;                               // option "pair_presum" (fp32 only; falls back when the tables do not fit)
-    void *d_widen = nullptr; size_t widen_bytes = 0;   // uint16 copy of a uint8 input (allocated on first use)
+    int dedisp_kernel = 0;            // option "dedisp_kernel": 0 auto, 1 direct, 2 rows
+    int group_size = 0;               // option "group_size": channels per pre-summed group, 0 = chosen by the cost model
+    RowsTables rows_f32, rows_u8;
+    void *d_scratch_f32 = nullptr, *d_scratch_u8 = nullptr;     // pre-summed rows [slots][nyrows][ystride] (mdsm_plan_reserve)
+    int scratch_slots_f32 = 0, scratch_slots_u8 = 0;            // beams the scratch holds at a time
+    size_t scratch_bytes_f32 = 0, scratch_bytes_u8 = 0;
 
     // host pipeline workspace (allocated on first mdsm_pipeline_host)
     void *ws_in = nullptr; size_t ws_in_bytes = 0;
@@ -92,10 +89,10 @@ int mdsm_launch_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int nb, int
                      double k_spec, uint8_t *d_chan_mask, uint8_t *d_spec_mask, cudaStream_t st);
 int mdsm_launch_dedisperse_direct(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
                                   cudaStream_t st);
-int mdsm_launch_dedisperse_tiled(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
-                                 cudaStream_t st);
-int mdsm_tiled_build_tables(mdsm_plan *p);
-int mdsm_tiled_num_geoms(int dtype);
-void mdsm_tiled_free_tables(mdsm_plan *p);
+int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
+                                cudaStream_t st);
+int mdsm_rows_build_tables(mdsm_plan *p);
+void mdsm_rows_free_tables(mdsm_plan *p);
+size_t mdsm_rows_scratch_bytes_per_beam(const mdsm_plan *p, int dtype);
 int mdsm_launch_detect(mdsm_plan *p, const void *d_out, int dtype, int beam0, int nb, double snr_thresh,
                        mdsm_event *d_events, int64_t max_events, unsigned long long *d_count, cudaStream_t st);

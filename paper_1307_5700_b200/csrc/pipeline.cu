@@ -30,9 +30,16 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
     MDSM_REQUIRE(window >= 0 && (window == 0 || p->nsamps % window == 0), "window must be 0 (no clip) or divide nsamps");
     if (nstreams < 1) nstreams = 1;
     if (nstreams > p->nbeams) nstreams = p->nbeams;
+    int rc;
+    if (p->dedisp_kernel != 1) {
+        // scratch of the dedispersion kernel (no-op once reserved).  Beam groups on different streams may only run
+        // side by side when every beam has its own scratch slot; otherwise the whole chain goes through one stream.
+        if ((rc = mdsm_plan_reserve(p, dtype, 0))) return rc;
+        const int slots = dtype == MDSM_F32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
+        if (slots > 0 && slots < p->nbeams) nstreams = 1;
+    }
     const size_t esize = dtype == MDSM_F32 ? 4 : 1;
     const size_t beam_in = (size_t)p->nchans * p->nsamps * esize;
-    int rc;
     if ((rc = ensure(&p->ws_in, &p->ws_in_bytes, beam_in * p->nbeams))) return rc;
     if ((rc = ensure(&p->ws_out, &p->ws_out_bytes, (size_t)p->nbeams * p->ndms * p->nsamps * 4))) return rc;
     const bool post = dtype == MDSM_F32 && (p->post_median_window > 1 || p->post_detrend);
@@ -53,35 +60,44 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
         MDSM_CUDA_TRY(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         p->ws_done.push_back(ev);
     }
+    // everything that enqueues work runs inside this lambda: on an error the copies from the caller's h_in and the kernels
+    // already in flight are waited for before returning, so that the caller may free or reuse its buffers
+    auto enqueue = [&]() -> int {
     // the counter is zeroed on stream 0; the other streams wait for that before their first detect
-    MDSM_CUDA_TRY(cudaMemsetAsync(p->ws_count, 0, sizeof(unsigned long long), p->ws_streams[0]));
-    MDSM_CUDA_TRY(cudaEventRecord(p->ws_done[0], p->ws_streams[0]));
-    for (int s = 1; s < nstreams; ++s) MDSM_CUDA_TRY(cudaStreamWaitEvent(p->ws_streams[s], p->ws_done[0], 0));
+        MDSM_CUDA_TRY(cudaMemsetAsync(p->ws_count, 0, sizeof(unsigned long long), p->ws_streams[0]));
+        MDSM_CUDA_TRY(cudaEventRecord(p->ws_done[0], p->ws_streams[0]));
+        for (int s = 1; s < nstreams; ++s) MDSM_CUDA_TRY(cudaStreamWaitEvent(p->ws_streams[s], p->ws_done[0], 0));
 
-    // contiguous beam groups, one per stream: whole groups per launch keep the persistent dedispersion grid full
-    // (one beam is only ~7 waves of tiles), while group g+1's copy still overlaps group g's kernels
-    const int per = (p->nbeams + nstreams - 1) / nstreams;
-    for (int b = 0, g = 0; b < p->nbeams; b += per, ++g) {
-        cudaStream_t st = p->ws_streams[g % nstreams];
-        const int nb = b + per <= p->nbeams ? per : p->nbeams - b;
-        MDSM_CUDA_TRY(cudaMemcpyAsync((char *)p->ws_in + beam_in * b, (const char *)h_in + beam_in * b, beam_in * nb,
-                                      cudaMemcpyHostToDevice, st));
-        if (window > 0 && (rc = mdsm_rfi_clip(p, p->ws_in, dtype, b, nb, window, k_chan, k_spec, nullptr, nullptr, st))) return rc;
-        if ((rc = mdsm_dedisperse(p, p->ws_in, dtype, b, nb, p->ws_out, st))) return rc;
-        const void *series = p->ws_out;
-        if (post) {                      // the paper's optional post-processing stage, fp32 series only
-            if (p->post_median_window > 1) {
-                if ((rc = mdsm_median_filter(p, (const float *)p->ws_out, (float *)p->ws_filt, b, nb, p->post_median_window, st))) return rc;
-                series = p->ws_filt;
+        // contiguous beam groups, one per stream: whole groups per launch keep the persistent dedispersion grid full
+        // (one beam is only ~7 waves of tiles), while group g+1's copy still overlaps group g's kernels
+        const int per = (p->nbeams + nstreams - 1) / nstreams;
+        for (int b = 0, g = 0; b < p->nbeams; b += per, ++g) {
+            cudaStream_t st = p->ws_streams[g % nstreams];
+            const int nb = b + per <= p->nbeams ? per : p->nbeams - b;
+            MDSM_CUDA_TRY(cudaMemcpyAsync((char *)p->ws_in + beam_in * b, (const char *)h_in + beam_in * b, beam_in * nb,
+                                          cudaMemcpyHostToDevice, st));
+            if (window > 0 && (rc = mdsm_rfi_clip(p, p->ws_in, dtype, b, nb, window, k_chan, k_spec, nullptr, nullptr, st))) return rc;
+            if ((rc = mdsm_dedisperse(p, p->ws_in, dtype, b, nb, p->ws_out, st))) return rc;
+            const void *series = p->ws_out;
+            if (post) {                      // the paper's optional post-processing stage, fp32 series only
+                if (p->post_median_window > 1) {
+                    if ((rc = mdsm_median_filter(p, (const float *)p->ws_out, (float *)p->ws_filt, b, nb, p->post_median_window, st))) return rc;
+                    series = p->ws_filt;
+                }
+                if (p->post_detrend && (rc = mdsm_detrend(p, (float *)series, b, nb, nullptr, st))) return rc;
             }
-            if (p->post_detrend && (rc = mdsm_detrend(p, (float *)series, b, nb, nullptr, st))) return rc;
+            if ((rc = mdsm_detect(p, series, dtype, b, nb, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
         }
-        if ((rc = mdsm_detect(p, series, dtype, b, nb, snr_thresh, p->ws_events, max_events, p->ws_count, st))) return rc;
-    }
-    // join every stream into stream 0, then read back the count and the events
-    for (int s = 1; s < nstreams; ++s) {
-        MDSM_CUDA_TRY(cudaEventRecord(p->ws_done[s], p->ws_streams[s]));
-        MDSM_CUDA_TRY(cudaStreamWaitEvent(p->ws_streams[0], p->ws_done[s], 0));
+        // join every stream into stream 0, then read back the count and the events
+        for (int s = 1; s < nstreams; ++s) {
+            MDSM_CUDA_TRY(cudaEventRecord(p->ws_done[s], p->ws_streams[s]));
+            MDSM_CUDA_TRY(cudaStreamWaitEvent(p->ws_streams[0], p->ws_done[s], 0));
+        }
+        return MDSM_OK;
+    };
+    if ((rc = enqueue()) != MDSM_OK) {
+        for (cudaStream_t s : p->ws_streams) cudaStreamSynchronize(s);
+        return rc;
     }
     unsigned long long cnt = 0;
     MDSM_CUDA_TRY(cudaMemcpyAsync(&cnt, p->ws_count, sizeof(cnt), cudaMemcpyDeviceToHost, p->ws_streams[0]));

@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <new>
 
 #include "mdsm_internal.h"
@@ -111,7 +112,7 @@ extern "C" mdsm_plan *mdsm_plan_create(int nbeams, int nchans, double f_top, dou
             ok = false;
         }
     }
-    if (ok && mdsm_tiled_build_tables(p) != MDSM_OK) ok = false;
+    if (ok && mdsm_rows_build_tables(p) != MDSM_OK) ok = false;
     if (!ok) {
         mdsm_plan_destroy(p);
         return nullptr;
@@ -129,7 +130,9 @@ extern "C" void mdsm_plan_destroy(mdsm_plan *p)
     cudaFree(p->d_spec_part_u);
     cudaFree(p->d_series_stats);
     cudaFree(p->ws_filt);
-    mdsm_tiled_free_tables(p);
+    mdsm_rows_free_tables(p);
+    cudaFree(p->d_scratch_f32);
+    cudaFree(p->d_scratch_u8);
     cudaFree(p->ws_in);
     cudaFree(p->ws_out);
     cudaFree(p->ws_events);
@@ -150,23 +153,30 @@ extern "C" int mdsm_plan_get_delays(const mdsm_plan *p, int32_t *h_delays)
     return MDSM_OK;
 }
 
+static void drop_scratch(mdsm_plan *p)
+{
+    cudaFree(p->d_scratch_f32);
+    cudaFree(p->d_scratch_u8);
+    p->d_scratch_f32 = p->d_scratch_u8 = nullptr;
+    p->scratch_slots_f32 = p->scratch_slots_u8 = 0;
+    p->scratch_bytes_f32 = p->scratch_bytes_u8 = 0;
+}
+
 extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value)
 {
     MDSM_REQUIRE(p && key, "null argument");
     if (strcmp(key, "dedisp_kernel") == 0) {
-        MDSM_REQUIRE(value >= 0 && value <= 2, "dedisp_kernel must be 0 (auto), 1 (direct) or 2 (tiled)");
+        MDSM_REQUIRE(value >= 0 && value <= 2, "dedisp_kernel must be 0 (auto), 1 (direct) or 2 (pre-summed rows)");
         p->dedisp_kernel = (int)value;
         return MDSM_OK;
     }
-    if (strcmp(key, "pair_presum_u8") == 0) {
-        MDSM_REQUIRE(value == 0 || value == 1, "pair_presum_u8 must be 0 or 1");
-        p->pair_presum_u8 = (int)value;
-        return mdsm_tiled_build_tables(p);
-    }
-    if (strcmp(key, "pair_presum") == 0) {
-        MDSM_REQUIRE(value == 0 || value == 1, "pair_presum must be 0 or 1");
-        p->pair_presum = (int)value;
-        return mdsm_tiled_build_tables(p);
+    if (strcmp(key, "group_size") == 0) {
+        MDSM_REQUIRE(value >= 0 && value <= 8, "group_size must be 0 (chosen by the plan) or 1..8 channels");
+        // the tables and the scratch layout change: wait for whatever still uses them, then drop the reservation
+        MDSM_CUDA_TRY(cudaDeviceSynchronize());
+        drop_scratch(p);
+        p->group_size = (int)value;
+        return mdsm_rows_build_tables(p);
     }
     if (strcmp(key, "post_median_window") == 0) {
         MDSM_REQUIRE(value == 0 || (value >= 1 && value <= 33 && (value & 1)), "post_median_window must be 0 (off) or odd and <= 33");
@@ -177,12 +187,6 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
         MDSM_REQUIRE(value == 0 || value == 1, "post_detrend must be 0 or 1");
         p->post_detrend = (int)value;
         return MDSM_OK;
-    }
-    if (strcmp(key, "tiled_geom_f32") == 0 || strcmp(key, "tiled_geom_u8") == 0) {
-        const bool f = key[11] == 'f';
-        MDSM_REQUIRE(value >= -1 && value < mdsm_tiled_num_geoms(f ? MDSM_F32 : MDSM_U8), "no such tile geometry (-1 = automatic)");
-        (f ? p->tiled_geom_f32 : p->tiled_geom_u8) = (int)value;
-        return mdsm_tiled_build_tables(p);
     }
     mdsm_set_error("unknown option '%s'", key);
     return MDSM_EINVAL;
@@ -195,6 +199,9 @@ static int check_common(const mdsm_plan *p, const void *ptr, int dtype, int beam
     MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
     MDSM_REQUIRE(beam0 >= 0 && nb >= 1 && beam0 + nb <= p->nbeams, "beam range [%d, %d) outside [0, %d)", beam0,
                  beam0 + nb, p->nbeams);
+    int dev = -1;
+    MDSM_CUDA_TRY(cudaGetDevice(&dev));
+    MDSM_REQUIRE(dev == p->device, "the plan belongs to device %d, the current device is %d", p->device, dev);
     return MDSM_OK;
 }
 
@@ -215,12 +222,70 @@ extern "C" int mdsm_dedisperse(mdsm_plan *p, const void *d_in, int dtype, int be
     int rc = check_common(p, d_in, dtype, beam0, nb);
     if (rc) return rc;
     MDSM_REQUIRE(d_out, "null output pointer");
-    const TiledTables &tt = dtype == MDSM_F32 ? p->tiled_f32 : p->tiled_u8;
-    bool tiled_ok = tt.ok && ((uintptr_t)d_in % 16 == 0) && ((uintptr_t)d_out % 16 == 0);
-    if (p->dedisp_kernel == 2) MDSM_REQUIRE(tiled_ok, "tiled kernel unavailable for this shape/alignment");
-    if (p->dedisp_kernel == 1 || !tiled_ok)
+    const RowsTables &rt = dtype == MDSM_F32 ? p->rows_f32 : p->rows_u8;
+    if (p->dedisp_kernel == 1 || (p->dedisp_kernel == 0 && !rt.ok))
         return mdsm_launch_dedisperse_direct(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
-    return mdsm_launch_dedisperse_tiled(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
+    MDSM_REQUIRE(rt.ok, "the pre-summed-rows kernel has no tables for this plan (see mdsm_plan_kernel_info)");
+    MDSM_REQUIRE(dtype == MDSM_F32 ? p->d_scratch_f32 != nullptr : p->d_scratch_u8 != nullptr,
+                 "dedispersion scratch not reserved: call mdsm_plan_reserve(plan, dtype, 0) once before mdsm_dedisperse");
+    return mdsm_launch_dedisperse_rows(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int mdsm_plan_reserve(mdsm_plan *p, int dtype, int64_t max_bytes)
+{
+    MDSM_REQUIRE(p, "null plan");
+    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
+    MDSM_REQUIRE(max_bytes >= 0, "max_bytes must be >= 0 (0 = default)");
+    const bool f32 = dtype == MDSM_F32;
+    const size_t per_beam = mdsm_rows_scratch_bytes_per_beam(p, dtype);
+    if (per_beam == 0) return MDSM_OK;                       // this plan runs the direct kernel: nothing to reserve
+    void *&scratch = f32 ? p->d_scratch_f32 : p->d_scratch_u8;
+    int &slots = f32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
+    size_t &bytes = f32 ? p->scratch_bytes_f32 : p->scratch_bytes_u8;
+    size_t limit = (size_t)max_bytes;
+    if (limit == 0) {
+        size_t free_b = 0, total_b = 0;
+        MDSM_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
+        limit = free_b / 4;                                   // default: at most a quarter of what is free now
+    }
+    int want = (int)std::min<size_t>((size_t)p->nbeams, limit / per_beam);
+    if (want < 1) want = 1;
+    if (scratch && slots == want) return MDSM_OK;
+    if (scratch) {
+        MDSM_CUDA_TRY(cudaDeviceSynchronize());
+        cudaFree(scratch);
+        scratch = nullptr; slots = 0; bytes = 0;
+    }
+    const cudaError_t e = cudaMalloc(&scratch, per_beam * (size_t)want);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        scratch = nullptr;
+        mdsm_set_error("mdsm_plan_reserve: cudaMalloc(%zu bytes for %d beams of pre-summed rows) failed: %s", per_beam * (size_t)want,
+                       want, cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? MDSM_ENOMEM : MDSM_ECUDA;
+    }
+    slots = want;
+    bytes = per_beam * (size_t)want;
+    return MDSM_OK;
+}
+
+extern "C" int mdsm_plan_kernel_info(const mdsm_plan *p, int dtype, char *buf, int64_t buflen)
+{
+    MDSM_REQUIRE(p && buf && buflen > 0, "null argument");
+    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
+    const bool f32 = dtype == MDSM_F32;
+    const RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
+    const bool rows = p->dedisp_kernel != 1 && rt.ok;
+    if (!rows) {
+        snprintf(buf, (size_t)buflen, "kernel=direct reason=%s", p->dedisp_kernel == 1 ? "option" : "no_tables");
+        return 0;
+    }
+    snprintf(buf, (size_t)buflen,
+             "kernel=rows group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%d row_slots=%d row_pitch=%d stages=%d "
+             "smem_bytes=%zu nyrows=%d rows_per_block=%.0f scratch_slots=%d scratch_bytes=%zu",
+             rt.G, rt.DB, rt.stride, rt.Q, rt.CS, rt.pitch, rt.stages, rt.smem_bytes, rt.nyrows, rt.rows_per_block,
+             f32 ? p->scratch_slots_f32 : p->scratch_slots_u8, f32 ? p->scratch_bytes_f32 : p->scratch_bytes_u8);
+    return 1;
 }
 
 extern "C" int mdsm_detect(mdsm_plan *p, const void *d_out, int dtype, int beam0, int nb, double snr_thresh,

@@ -12,7 +12,9 @@ def torch_cuda():
 class Plan:
     """RAII wrapper used by tests only."""
 
-    def __init__(self, cfg_or_args):
+    def __init__(self, cfg_or_args, scratch_limit=0):
+        self.reserved = set()
+        self.scratch_limit = scratch_limit
         import paper_1307_5700_b200 as m
         self.m = m
         args = cfg_or_args.plan_args() if hasattr(cfg_or_args, "plan_args") else tuple(cfg_or_args)
@@ -33,6 +35,14 @@ class Plan:
     def __exit__(self, *a):
         self.close()
 
+    def info(self, dtype):
+        return self.m.mdsm_plan_kernel_info(self.h, dtype)
+
+    def set_option(self, key, value):
+        self.m.mdsm_plan_set_option(self.h, key, value)
+        if key == "group_size":
+            self.reserved.clear()          # the option drops the reservation
+
     def delays(self):
         return self.m.mdsm_plan_get_delays(self.h, self.ndms, self.nchans)
 
@@ -43,6 +53,10 @@ class Plan:
         if out is None:
             out = torch.full((self.nbeams, self.ndms, self.nsamps), -7, dtype=odt, device="cuda")
         self.m.mdsm_plan_set_option(self.h, "dedisp_kernel", kernel)
+        dtype = self.m.MDSM_F32 if d_in.dtype == torch.float32 else self.m.MDSM_U8
+        if kernel != 1 and dtype not in self.reserved:
+            self.m.mdsm_plan_reserve(self.h, dtype, self.scratch_limit)
+            self.reserved.add(dtype)
         self.m.mdsm_dedisperse(self.h, d_in, beam0, nb, out)
         torch.cuda.synchronize()
         return out

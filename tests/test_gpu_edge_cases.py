@@ -92,9 +92,10 @@ def test_no_events_constant_input_and_argument_errors():
             m.mdsm_plan_create(*bad)
 
 
-def test_coarse_dm_grid_selects_a_narrower_tile_geometry():
-    """dm_step = 0.3: three times the delay spread per DM step of the BEST-2 grid.  The automatic geometry choice must
-    still find a tiled fp32 kernel (fewer DMs per warp); whatever runs must match the oracle."""
+def test_coarse_dm_grid_still_runs_the_rows_kernel():
+    """dm_step = 0.3: three times the delay spread per DM step of the BEST-2 grid, so a channel group takes many more
+    delay patterns.  The plan's cost model must still find a group size whose tables fit the kernel (kernel=2 errors
+    otherwise); whatever it picks must match the oracle."""
     torch = _torch()
     args = (2, 256, 418.0, -20.0 / 256, 51.2e-6, 16384, 0.0, 0.3, 60)
     g = np.random.default_rng(8)
@@ -102,11 +103,12 @@ def test_coarse_dm_grid_selects_a_narrower_tile_geometry():
     xf = g.normal(size=(2, 256, 16384)).astype(np.float32)
     xu = g.integers(0, 256, size=(2, 256, 16384)).astype(np.uint8)
     with Plan(args) as p:
+        assert p.info(0)["kernel"] == "rows" and p.info(1)["kernel"] == "rows"
         ref, ab = oracle.dedisperse(xf, d)
-        got = out_to_numpy(p.dedisperse(torch.from_numpy(xf).cuda(), kernel=2), p.nsamps_out)      # tiled, not direct
+        got = out_to_numpy(p.dedisperse(torch.from_numpy(xf).cuda(), kernel=2), p.nsamps_out)
         assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)
         refu, _ = oracle.dedisperse(xu, d)
-        gotu = out_to_numpy(p.dedisperse(torch.from_numpy(xu).cuda(), kernel=0), p.nsamps_out)
+        gotu = out_to_numpy(p.dedisperse(torch.from_numpy(xu).cuda(), kernel=2), p.nsamps_out)
         assert np.array_equal(gotu, refu)
 
 
@@ -126,11 +128,13 @@ def test_fp32_same_sign_data_stays_inside_the_tolerance_at_4096_channels():
         assert ratio.max() < 0.7, ratio.max()              # measured 0.42 / 0.44: a factor two of margin
 
 
-def test_pair_presum_falls_back_when_its_scratch_does_not_fit():
-    """With device memory nearly full the fp32 path must go on without the pre-summed copy, not fail."""
+def test_dedisperse_refuses_to_run_unreserved_and_reserve_reports_out_of_memory():
+    """nothing is allocated per call.  The scratch of the rows kernel comes from mdsm_plan_reserve; without
+    it mdsm_dedisperse returns MDSM_EINVAL (it never allocates or falls back silently), and a reservation that does not
+    fit returns MDSM_ENOMEM and leaves the plan usable."""
     torch = _torch()
     import paper_1307_5700_b200 as m
-    args = (1, 256, 418.0, -20.0 / 256, 51.2e-6, 1 << 17, 0.0, 0.1, 64)         # pair scratch ~ 2 x 134 MB
+    args = (1, 256, 418.0, -20.0 / 256, 51.2e-6, 1 << 17, 0.0, 0.1, 64)
     g = np.random.default_rng(12)
     x = g.normal(size=(1, 256, 1 << 17)).astype(np.float32)
     d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
@@ -138,17 +142,138 @@ def test_pair_presum_falls_back_when_its_scratch_does_not_fit():
     with Plan(args) as p:
         dx = torch.from_numpy(x).cuda()
         out = torch.full((1, 64, 1 << 17), -7, dtype=torch.float32, device="cuda")
+        with pytest.raises(m.MdsmError) as ei:
+            m.mdsm_dedisperse(p.h, dx, 0, 1, out)
+        assert ei.value.status == m.MDSM_EINVAL and "mdsm_plan_reserve" in str(ei.value)
+        need = p.info(0)["nyrows"] * (1 << 17) * 4
         torch.cuda.synchronize()
         torch.cuda.empty_cache()
         free, _ = torch.cuda.mem_get_info()
-        hog = torch.empty((max(free - (96 << 20), 0),), dtype=torch.uint8, device="cuda")   # leave 96 MB
+        hog = torch.empty((max(free - need // 2, 0),), dtype=torch.uint8, device="cuda")   # leave half of what one beam needs
         try:
-            l0 = m.mdsm_plan_launch_count(p.h)
-            m.mdsm_dedisperse(p.h, dx, 0, 1, out)
-            torch.cuda.synchronize()
-            assert m.mdsm_plan_launch_count(p.h) - l0 == 1                      # no pre-pass launch: plain tiled kernel
+            with pytest.raises(m.MdsmError) as ei:
+                m.mdsm_plan_reserve(p.h, m.MDSM_F32, 0)
+            assert ei.value.status == m.MDSM_ENOMEM
         finally:
             del hog
             torch.cuda.empty_cache()
+        m.mdsm_plan_reserve(p.h, m.MDSM_F32, 0)
+        assert p.info(0)["scratch_slots"] == 1 and p.info(0)["scratch_bytes"] == need
+        m.mdsm_dedisperse(p.h, dx, 0, 1, out)
+        torch.cuda.synchronize()
         got = out_to_numpy(out, p.nsamps_out)
         assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.uint8])
+def test_stage_calls_neither_allocate_nor_synchronise(dtype):
+    """SURVEY 8(b) "nothing is allocated per call ... no host sync inside": after mdsm_plan_reserve the three stage calls are
+    captured into a CUDA graph on a side stream (stream capture fails on any synchronisation or cudaMalloc), free device
+    memory does not change, and replaying the graph reproduces the result of the direct calls bit for bit."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    args = (3, 128, 418.0, -20.0 / 128, 51.2e-6, 8192, 0.0, 0.1, 70)
+    g = np.random.default_rng(21)
+    x = g.normal(5.0, 1.0, size=(3, 128, 8192)).astype(np.float32) if dtype == np.float32 else g.integers(0, 256, size=(3, 128, 8192)).astype(np.uint8)
+    mdt = m.MDSM_F32 if dtype == np.float32 else m.MDSM_U8
+    with Plan(args) as p:
+        m.mdsm_plan_reserve(p.h, mdt, 0)
+        pristine = torch.from_numpy(x).cuda()
+        work = pristine.clone()
+        odt = torch.float32 if dtype == np.float32 else torch.int32
+        out = torch.zeros((3, 70, 8192), dtype=odt, device="cuda")
+        ev = torch.zeros((1 << 16, 4), dtype=torch.int32, device="cuda")
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+
+        def chain(stream):
+            m.mdsm_rfi_clip(p.h, work, 0, 3, 64, 5.0, 5.0, None, None, stream)
+            m.mdsm_dedisperse(p.h, work, 0, 3, out, stream)
+            m.mdsm_detect(p.h, out, 0, 3, 4.0, ev, 1 << 16, cnt, stream, dtype=mdt)
+
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            chain(side)                                        # warm-up outside the capture (lazy module loading)
+        side.synchronize()
+        work.copy_(pristine); out.zero_(); cnt.zero_()
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        chain(side)                                            # the plain calls: device memory must not move
+        side.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        assert free1 == free0
+        ref_out, ref_cnt = out.clone(), int(cnt.item())
+        work.copy_(pristine); out.zero_(); cnt.zero_()
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):             # raises if a call synchronises or allocates
+            chain(side)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref_out) and int(cnt.item()) == ref_cnt and ref_cnt > 0
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.uint8])
+def test_scratch_smaller_than_the_plan_walks_the_beams_through_it(dtype):
+    """A reservation for fewer beams than the plan holds (config 5 on a full device): mdsm_dedisperse takes the beams
+    through the scratch slots in stream order, for any beam0/nb, and mdsm_pipeline_host keeps to one stream."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    args = (5, 96, 418.0, -20.0 / 96, 51.2e-6, 4096, 0.0, 0.1, 40)
+    g = np.random.default_rng(33)
+    x = g.normal(size=(5, 96, 4096)).astype(np.float32) if dtype == np.float32 else g.integers(0, 256, size=(5, 96, 4096)).astype(np.uint8)
+    d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
+    ref, ab = oracle.dedisperse(x, d)
+    mdt = m.MDSM_F32 if dtype == np.float32 else m.MDSM_U8
+    with Plan(args) as p:
+        per_beam = p.info(mdt)["nyrows"] * 4096 * (4 if dtype == np.float32 else 2)
+        m.mdsm_plan_reserve(p.h, mdt, 2 * per_beam + 100)
+        assert p.info(mdt)["scratch_slots"] == 2
+        p.reserved.add(mdt)
+        dx = torch.from_numpy(x).cuda()
+        out = p.dedisperse(dx, kernel=2)
+        p.dedisperse(dx, beam0=1, nb=3, kernel=2, out=out)                 # again, an odd sub-range
+        got = out_to_numpy(out, p.nsamps_out)
+        if dtype == np.float32:
+            assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)
+        else:
+            assert np.array_equal(got, ref)
+        # the host pipeline on top of the small scratch
+        ev_o, cnt_o, _ = oracle.detect(ref if dtype == np.uint8 else got.astype(np.float64), p.nsamps_out, 4.0)
+        h_ev = np.zeros(1 << 16, dtype=m.EVENT_DTYPE)
+        rc, cnt = m.mdsm_pipeline_host(p.h, x, 0, 0.0, 0.0, 4.0, h_ev, 1 << 16, 4)
+        assert rc == m.MDSM_OK and abs(cnt - cnt_o) <= (0 if dtype == np.uint8 else 3)
+
+
+@pytest.mark.parametrize("G", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_every_group_size_matches_the_oracle(G):
+    """Plan option group_size: every compiled pre-sum width, both dtypes, on a shape with a ragged last group (nchans not
+    a multiple of G for most G), several 256-channel parts, a ragged DM block and unaligned rows (odd nsamps)."""
+    torch = _torch()
+    args = (2, 601, 418.0, -20.0 / 601, 51.2e-6, 6001, 0.0, 0.05, 83)
+    g = np.random.default_rng(40 + G)
+    d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
+    xf = g.normal(size=(2, 601, 6001)).astype(np.float32)
+    xu = g.integers(0, 256, size=(2, 601, 6001)).astype(np.uint8)
+    with Plan(args) as p:
+        p.set_option("group_size", G)
+        for mdt in (0, 1):
+            info = p.info(mdt)
+            assert info["kernel"] == "rows" and info["group_size"] == G, info
+        ref, ab = oracle.dedisperse(xf, d)
+        got = out_to_numpy(p.dedisperse(torch.from_numpy(xf).cuda(), kernel=2), p.nsamps_out)
+        assert np.all(np.abs(got - ref) <= 1e-5 * ab + 1e-6)
+        refu, _ = oracle.dedisperse(xu, d)
+        outu = p.dedisperse(torch.from_numpy(xu).cuda(), kernel=2)
+        assert np.array_equal(out_to_numpy(outu, p.nsamps_out), refu)
+        assert (outu[:, :, p.nsamps_out:] == -7).all()                       # nothing past nsamps_out is touched
+
+
+def test_kernel_info_reports_the_direct_kernel_and_its_reason():
+    import paper_1307_5700_b200 as m
+    args = (1, 64, 418.0, -0.3125, 51.2e-6, 4096, 0.0, 0.1, 32)
+    with Plan(args) as p:
+        assert p.info(m.MDSM_F32)["kernel"] == "rows"
+        p.set_option("dedisp_kernel", 1)
+        info = p.info(m.MDSM_U8)
+        assert info["kernel"] == "direct" and info["reason"] == "option"

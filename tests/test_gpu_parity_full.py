@@ -4,8 +4,10 @@
 cfg 2, 3, 4: every output element of every beam is compared with the oracle (beam by beam, so the
 fp64 reference of one beam is all that is resident); clip masks, the clipped input and the event
 lists are compared too (bit-exact for u8, guard-banded for f32: readings B-ix, D-vi of DESIGN.md).
-cfg 5 (34 GB in, 17 GB out): the oracle computes a seeded sample of (beam, DM) series one by one
-(`oracle.dedisperse_rows`), plus the clip of one whole beam; detection is checked on the sampled series.
+cfg 5 (34 GB in, 17 GB out): every one of the 2048 series of beam 0 is compared element by element, plus a seeded
+sample of (beam, DM) series of two other beams (`oracle.dedisperse_rows` computes series one by one), plus the clip of
+one whole beam; detection is checked on the compared series.  Two more plans put the element offsets of the
+checked beam beyond 2^32 (4096 channels, fp32 and uint8).
 """
 import numpy as np
 import pytest
@@ -146,10 +148,13 @@ def test_cfg5_sampled_series():
                 xo = xg[None]
             else:
                 xo = dx[b].cpu().numpy()[None]                # clipped data as the GPU left it
-            ds = np.unique(np.concatenate([[0, 1, cfg.ndms - 1, cfg.ndms - 2], g.integers(0, cfg.ndms, size=8)]))
+            if b == check_beams[0]:                           # one whole beam: all 2048 series, element by element
+                ds = np.arange(cfg.ndms)
+            else:
+                ds = np.unique(np.concatenate([[0, 1, cfg.ndms - 1, cfg.ndms - 2], g.integers(0, cfg.ndms, size=8)]))
             ref, ab = oracle.dedisperse_rows(xo, delays, ds.astype(np.int64))
             got = out[b, torch.from_numpy(ds).cuda(), :nso].cpu().numpy()
-            _f32_check(got, ref, ab, f"beam {b} sampled series")
+            _f32_check(got, ref, ab, f"beam {b} series")
             # detection on the sampled series: per-series statistics make each series independent
             ev_o, cnt_o, _ = oracle.detect(np.ascontiguousarray(ref[None]), nso, cfg.snr_thresh)
             ev_o = ev_o.copy()
@@ -159,3 +164,40 @@ def test_cfg5_sampled_series():
             compare_events_f32(sel, ev_o, cfg.snr_thresh)
         tail = out[:, :, nso:]
         assert bool((tail == -7).all())
+
+
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_4096_channels_with_element_offsets_beyond_2_to_32(dtype):
+    """A 4096-channel plan whose last beam starts past 2^32 elements of the input (and, for the pre-summed rows, of the
+    scratch): all series of the LAST beam against the oracle.  The other beams are device-generated filler."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    nbeams, nchans, nsamps, ndms = (3, 4096, 532480, 24) if dtype == "f32" else (4, 4096, 360448, 24)
+    args = (nbeams, nchans, 418.0, -20.0 / nchans, 51.2e-6, nsamps, 150.0, 0.1, ndms)
+    assert (nbeams - 1) * nchans * nsamps > 2 ** 32
+    delays = oracle.delay_table(nchans, 418.0, -20.0 / nchans, 51.2e-6, 150.0, 0.1, ndms)
+    g = np.random.default_rng(77)
+    last = nbeams - 1
+    with Plan(args) as p:
+        nso = p.nsamps_out
+        if dtype == "f32":
+            dx = torch.empty((nbeams, nchans, nsamps), dtype=torch.float32, device="cuda")
+            dx.normal_(generator=torch.Generator(device="cuda").manual_seed(5))
+            xb = np.empty((nchans, nsamps), dtype=np.float32)
+            g.standard_normal(out=xb, dtype=np.float32)
+        else:
+            dx = torch.randint(0, 256, (nbeams, nchans, nsamps), dtype=torch.uint8, device="cuda",
+                               generator=torch.Generator(device="cuda").manual_seed(5))
+            xb = g.integers(0, 256, size=(nchans, nsamps), dtype=np.uint8)
+        dx[last].copy_(torch.from_numpy(xb))
+        out = p.dedisperse(dx, kernel=2)
+        info = p.info(m.MDSM_F32 if dtype == "f32" else m.MDSM_U8)
+        assert info["kernel"] == "rows"
+        ds = np.arange(ndms, dtype=np.int64)
+        ref, ab = oracle.dedisperse_rows(xb[None], delays, ds)
+        got = out[last, :, :nso].cpu().numpy()
+        if dtype == "f32":
+            _f32_check(got, ref, ab, "last beam")
+        else:
+            assert np.array_equal(got.view(np.uint32), ref)
+        assert bool((out[:, :, nso:] == -7).all())

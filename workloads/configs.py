@@ -174,3 +174,45 @@ def generate(cfg: Config, beams=None) -> np.ndarray:
     for i, b in enumerate(beams):
         out[i] = generate_beam(cfg, b)
     return out
+
+
+def generate_beam_device(cfg: Config, b: int, torch):
+    """One beam [nchans][nsamps] of cfg's recipe drawn ON THE DEVICE with a seeded torch.Generator (config 5
+    is generated on-device).  Same shapes, value distributions and injected structure as generate_beam, but another
+    random stream: bench.py times on it; parity tests use generate_beam, whose arrays reach the oracle too."""
+    gen = torch.Generator(device="cuda").manual_seed(cfg.seed + b)
+    x = torch.empty((cfg.nchans, cfg.nsamps), dtype=torch.float32, device="cuda")
+    x.normal_(generator=gen)
+    g = np.random.Generator(np.random.PCG64(np.random.SeedSequence([cfg.seed + b, 11])))
+    chan = torch.arange(cfg.nchans, device="cuda")
+
+    def inject(scale):
+        for (dm, t0, w, a) in pulses(cfg, b):
+            sw = torch.from_numpy(cfg.sweep(dm)).cuda()
+            for i in range(w):
+                t = t0 + sw + i
+                ok = t < cfg.nsamps
+                x[chan[ok], t[ok]] += scale * a
+
+    if cfg.recipe in ("cfg1", "cfg5"):
+        inject(1.0)
+        return x
+    if cfg.recipe == "cfg2":
+        inject(1.0)
+        gain = torch.from_numpy(g.uniform(0.5, 1.5, size=cfg.nchans).astype(np.float32)).cuda()
+        x *= gain[:, None]
+        return x
+    if cfg.recipe == "cfg4":
+        x.mul_(10.0).add_(64.0)
+        inject(10.0)
+        t = torch.arange(cfg.nsamps, dtype=torch.float64, device="cuda")
+        for c in g.choice(cfg.nchans, size=12, replace=False):
+            P = g.uniform(2000.0, 20000.0)
+            phi = g.uniform(0.0, 2 * np.pi)
+            x[int(c)] += (40.0 + 15.0 * torch.sin(2 * np.pi * t / P + phi)).float()
+        for _ in range(50):
+            ts = int(g.integers(0, cfg.nsamps - 3))
+            dur = int(g.integers(1, 4))
+            x[:, ts:ts + dur] += 80.0
+        return x.round_().clamp_(0.0, 255.0).to(torch.uint8)
+    raise ValueError(cfg.recipe)

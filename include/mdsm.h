@@ -15,8 +15,13 @@
  *   out [nbeams][ndms][nsamps]     float (MDSM_F32) or uint32_t (MDSM_U8); row stride = nsamps,
  *                                  only t < nsamps_out = nsamps - max_delay is written / valid
  *                                  (overlap reading A3: Eq. 6)
- * The device-pointer calls only enqueue work on `cuda_stream` (a cudaStream_t cast to void*;
- * NULL = the legacy default stream); they never synchronise and never allocate.
+ * The device-pointer stage calls (mdsm_rfi_clip, mdsm_dedisperse, mdsm_detect, the post-processing calls) only
+ * enqueue work on `cuda_stream` (a cudaStream_t cast to void*; NULL = the legacy default stream); they never
+ * synchronise and never allocate, so they can be captured into a CUDA graph.  Whatever device memory the path needs
+ * beyond the caller's buffers is allocated by mdsm_plan_create and mdsm_plan_reserve.
+ * Threads: a plan is NOT internally locked.  Calls on one plan must come from one host thread at a time (the paper's
+ * host model is one thread per beam: give every such thread its own plan, or serialise the calls);
+ * different plans are independent.  mdsm_last_error() is thread-local.
  * beam0/nb select a contiguous range of beams so that the host can drive beam groups on
  * different streams ("parallelized across beams"); pointers always address the
  * FULL [nbeams]... arrays, the call offsets them by beam0 itself.
@@ -66,7 +71,7 @@ const char *mdsm_last_error(void);
  *      mdsm_median_filter / mdsm_detrend on the fp32 series between dedispersion and detection (ignored for uint8).
  * Unknown key/value -> MDSM_EINVAL. */
 int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);
-/* Allocates the plan-owned scratch of mdsm_dedisperse for `dtype`: the exactly pre-summed channel-group rows
+/* Allocates the plan-owned scratch of mdsm_dedisperse for `dtype`: the pre-summed channel-group rows (uint8: exact; fp32: same terms, another order)
  * (DESIGN.md section 6.1), nyrows * nsamps * (4 | 2) bytes per beam.  Call once after mdsm_plan_create (and after
  * changing "group_size") and before the first mdsm_dedisperse of that dtype; mdsm_pipeline_host calls it itself.
  * max_bytes = 0: as many beams as fit a quarter of the free device memory; otherwise at most max_bytes (never less
@@ -103,11 +108,11 @@ int mdsm_rfi_clip(mdsm_plan *plan, void *d_in, int dtype, int beam0, int nb,
  * MDSM_F32: float in, float out (fp32 accumulation; |err| <= 1e-5 * sum_c|in| + 1e-6).
  * MDSM_U8 : uint8 in, uint32 out, exact.
  * d_in [nbeams][nchans][nsamps], d_out [nbeams][ndms][nsamps] (only t < nsamps_out of the rows of beams
- * [beam0, beam0+nb) is written), both caller-owned device buffers; 16-byte aligned buffers and nsamps % 4 == 0
- * (uint8: % 8) take the tiled kernels, anything else the direct kernel.  Asynchronous on cuda_stream.  The FIRST call
- * of a dtype allocates plan-owned scratch (uint8: a uint16 copy of the input; float: the pre-summed channel pairs,
- * about two input sizes -- if that does not fit, the plan synchronises the device once, drops the pair pre-sums and
- * goes on with the plain tiled kernel); later calls allocate nothing. */
+ * [beam0, beam0+nb) is written), both caller-owned device buffers of any alignment.  Asynchronous on cuda_stream;
+ * allocates nothing: the scratch of the pre-summed-rows kernel must have been reserved with
+ * mdsm_plan_reserve(plan, dtype, ...) -- MDSM_EINVAL otherwise.  A plan whose delay table the pre-summed-rows
+ * kernel cannot express runs the direct kernel (one thread per output; mdsm_plan_kernel_info says which and why).
+ * fp32: the channel groups are added first, so the summation order differs from the definition's (same terms). */
 int mdsm_dedisperse(mdsm_plan *plan, const void *d_in, int dtype, int beam0, int nb,
                     void *d_out, void *cuda_stream);
 

@@ -64,7 +64,9 @@ const char *mdsm_last_error(void);
 
 /* Plan options (synchronise the device; not for use while work of this plan is in flight).
  *  "dedisp_kernel": 0 = auto (the pre-summed-rows kernel whenever the plan has tables for it, else the direct kernel),
- *      1 = direct (one thread per output, global loads: the cross-check kernel), 2 = pre-summed rows or MDSM_EINVAL.
+ *      1 = direct (one thread per output, global loads: the cross-check kernel), 2 = pre-summed rows or MDSM_EINVAL,
+ *      3 = pre-summed rows with the operand windows staged in tensor memory (fp32 only; an experimental variant of the
+ *      main kernel, slower than 2 today -- DESIGN.md section 6.1) or MDSM_EINVAL.
  *  "group_size": channels per pre-summed group, 1..8, or 0 (default) = the plan's cost model picks it.  Changing it
  *      rebuilds the tables and DROPS the scratch reservation (call mdsm_plan_reserve again).
  *  "post_median_window" (0 = off, else odd <= 33) and "post_detrend" (0/1): mdsm_pipeline_host runs

@@ -418,6 +418,265 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
     }
 }
 
+// ------------------------------------------------------------------ step 2, TMEM variant (fp32)
+// The rows kernel above is bound by the shared-memory pipe: one 32-bit operand word per add, 32 words per clock and SM.
+// Tensor memory (TMEM, 128 lanes x 512 columns x 32 bit per SM) has its own read path into the register file
+// (tcgen05.ld), measured at ~3x that rate with the adds in the loop, and -- unlike registers -- its COLUMN address is
+// a run-time value.  So the operand window moves there:
+//   * TMEM lane l of a quadrant holds the samples  s0 + P l + [0, P + S)  of a staged y row in consecutive columns
+//     (P = outputs per lane and DM, S = spread of the window starts of the DMs that use the row);
+//   * a consumer thread (lane l) owns the P consecutive outputs  tile_t0 - sigma_d + P l + [0, P)  of each of its D DMs
+//     and fetches, per (DM, group), P consecutive columns at the DM's own column offset: one tcgen05.ld.32x32b.x16 per
+//     15 adds, no alignment cases, no shared-memory traffic;
+//   * a STAGER warp per quadrant (TMEM lanes are only reachable from the warps w with w % 4 == quadrant) copies each
+//     row the quadrant's 4 D DMs use from the TMA-filled shared-memory stage into TMEM: conflict-free 32-bit loads
+//     (P is odd) + tcgen05.st.  A staged word then serves every DM of the quadrant that uses the row, so the
+//     shared-memory pipe carries ~0.5 words per add instead of 1.
+// Warps: 16 consumers (quadrant = w & 3, D DMs each), 4 stagers (w = 16..19), 1 TMA producer (w = 20); the two non-consumer
+// warpgroups hand most of their registers to the consumers (setmaxnreg).
+// Rings: shared-memory stages (producer -> stagers), two TMEM stages of 256 columns (stager -> the quadrant's consumers).
+constexpr int kTmWarps = 24;         // 16 consumers + 4 stagers + the producer's warpgroup (3 of its warps idle)
+constexpr int kTmProducer = 20;
+constexpr int kTmCols = 256;          // TMEM columns per stage (two stages)
+constexpr int kTmQMax = 4;            // most groups per slab
+constexpr int kTmRQMax = 16;          // most staged rows per quadrant and slab
+
+struct TmemArgs {
+    const float *y;
+    float *out;
+    const int4 *rowdesc;              // [nblk][nslab_max][CS]: (y row or -1, first staged sample - tile_t0, samples, 0)
+    const uint32_t *tab;              // [nblk][nslab_max][tabw]
+    const int32_t *nslab;             // [nblk]
+    const int32_t *sigma;             // [DB]
+    int beam0, nslots, nyrows, ndms;
+    int nblk, ntile_t, nslab_max, CS, pitch, stages, tabw, span;
+    long long ntiles, nsamps, nsamps_out, ystride;
+};
+
+__device__ __forceinline__ void tm_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                   "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tm_st8(uint32_t taddr, const uint32_t (&r)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+}
+__device__ __forceinline__ void tm_st16(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+                 "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+                 "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+                 : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+template <int D, int P>
+__global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const TmemArgs a)
+{
+    static_assert(P % 2 == 1 && P <= 16, "P must be odd (conflict-free staging) and fit one x16 load");
+    constexpr int DQ = 4 * D, DB = 16 * D, TENT = DQ * kTmQMax + 4;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int stages = a.stages;
+    const uint32_t row_bytes = (uint32_t)a.pitch * 4u;
+    const uint32_t tab_bytes = (uint32_t)a.tabw * 4u;
+    const uint32_t stage_bytes = (a.CS * row_bytes + tab_bytes + 127u) & ~127u;
+    uint32_t *tent = reinterpret_cast<uint32_t *>(smem + (size_t)stages * stage_bytes);       // [2][4][TENT]
+    uint64_t *full = reinterpret_cast<uint64_t *>(tent + 2 * 4 * TENT);
+    uint64_t *empty = full + stages;
+    uint64_t *tfull = empty + stages;          // [2][4]
+    uint64_t *tempty = tfull + 8;              // [2][4]
+    uint32_t *tbase_slot = reinterpret_cast<uint32_t *>(tempty + 8);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    for (uint32_t i = threadIdx.x; i < stages * stage_bytes / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[s], 32);
+            mbar_init(&empty[s], 4);
+        }
+        for (int s = 0; s < 8; ++s) {
+            mbar_init(&tfull[s], 1);
+            mbar_init(&tempty[s], 4);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == kTmProducer) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tbase_slot)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tm_fence_before();
+    __syncthreads();
+    tm_fence_after();
+    const uint32_t tbase = *tbase_slot;
+    if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
+
+    if (warp > kTmProducer) {
+        // idle warps of the producer's warpgroup
+    } else if (warp == kTmProducer) {
+        // ===== TMA producer: lane r copies row r of every slab, lane 0 also the slab's table slice =====
+        int st = 0;
+        uint32_t ph = 1;
+        bool first_lap = true;
+        const uint32_t smem0 = smem_u32(smem);
+        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+            const int blk = (int)(tile % a.nblk);
+            const long long rest = tile / a.nblk;
+            const int tt = (int)(rest % a.ntile_t), bb = (int)(rest / a.ntile_t);
+            const long long tile_t0 = (long long)tt * a.span;
+            const float *ybeam = a.y + (size_t)((a.beam0 + bb) % a.nslots) * a.nyrows * (size_t)a.ystride;
+            const int4 *rd = a.rowdesc + (size_t)blk * a.nslab_max * a.CS;
+            const uint32_t *tb = a.tab + (size_t)blk * a.nslab_max * a.tabw;
+            const int nslab = a.nslab[blk];
+            int4 desc = lane < a.CS ? rd[lane] : make_int4(-1, 0, 0, 0);
+            for (int slab = 0; slab < nslab; ++slab) {
+                const int4 cur = desc;
+                if (slab + 1 < nslab && lane < a.CS) desc = rd[(size_t)(slab + 1) * a.CS + lane];
+                if (!first_lap) mbar_wait_sleep(&empty[st], ph);
+                const uint32_t sbase = smem0 + st * stage_bytes;
+                uint32_t bytes = 0;
+                long long lo = 0, g0 = 0;
+                if (cur.x >= 0) {
+                    g0 = tile_t0 + cur.y;
+                    lo = g0 < 0 ? 0 : g0;
+                    long long hi = g0 + cur.z;
+                    if (hi > a.ystride) hi = a.ystride;
+                    if (hi > lo) bytes = (uint32_t)((hi - lo) * 4);
+                }
+                mbar_arrive_expect_tx(&full[st], bytes + (lane == 0 ? tab_bytes : 0u));
+                if (bytes) bulk_g2s(sbase + lane * row_bytes + (uint32_t)((lo - g0) * 4), ybeam + (size_t)cur.x * a.ystride + lo, bytes, &full[st]);
+                if (lane == 0) bulk_g2s(sbase + a.CS * row_bytes, tb + (size_t)slab * a.tabw, tab_bytes, &full[st]);
+                if (++st == stages) { st = 0; ph ^= 1; first_lap = false; }
+            }
+        }
+    } else if (warp >= 16) {
+        // ===== stager of quadrant q: shared-memory stage -> TMEM stage =====
+        const int q = warp & 3;
+        const uint32_t tq = tbase + ((uint32_t)(q * 32) << 16);
+        int st = 0, ts = 0;
+        uint32_t ph = 0, tph = 1;
+        bool tfirst = true;
+        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+            const int nslab = a.nslab[(int)(tile % a.nblk)];
+            for (int slab = 0; slab < nslab; ++slab) {
+                mbar_wait(&full[st], ph);
+                const unsigned char *sbase = smem + (size_t)st * stage_bytes;
+                const uint32_t *tab = reinterpret_cast<const uint32_t *>(sbase + a.CS * row_bytes);
+                const int nr = (int)tab[q];
+                if (!tfirst) mbar_wait(&tempty[ts * 4 + q], tph);
+                tm_fence_after();
+                const float *rows = reinterpret_cast<const float *>(sbase) + P * lane;
+                const uint32_t tstage = tq + ts * kTmCols;
+#pragma unroll 1
+                for (int r = 0; r < nr; ++r) {
+                    const uint32_t soff = tab[8 + (q * kTmRQMax + r) * 2], w1 = tab[8 + (q * kTmRQMax + r) * 2 + 1];
+                    const float *src = rows + soff;
+                    const uint32_t tcol = tstage + (w1 & 0xffffu);
+                    const int n8 = (int)(w1 >> 16);
+                    int k = 0;
+#pragma unroll 1
+                    for (; k + 2 <= n8; k += 2) {                 // 16 columns per round: all the loads are in flight together
+                        uint32_t v[16];
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(src[8 * k + i]);
+                        tm_st16(tcol + 8 * k, v);
+                    }
+                    if (k < n8) {
+                        uint32_t v[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) v[i] = __float_as_uint(src[8 * k + i]);
+                        tm_st8(tcol + 8 * k, v);
+                    }
+                }
+                // the quadrant's entries (TMEM column per (DM, group)) and the number of groups of this slab
+                uint32_t *te = tent + (ts * 4 + q) * TENT;
+                const uint32_t *ent = tab + 8 + 4 * kTmRQMax * 2 + q * DQ * kTmQMax;
+                for (int i = lane; i < DQ * kTmQMax; i += 32) te[i] = ent[i];
+                if (lane == 0) te[DQ * kTmQMax] = tab[4];
+                tm_wait_st();
+                tm_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(&tfull[ts * 4 + q]);
+                    mbar_arrive(&empty[st]);
+                }
+                if (++st == stages) { st = 0; ph ^= 1; }
+                if (++ts == 2) { ts = 0; tph ^= 1; tfirst = false; }
+            }
+        }
+    } else {
+        // ===== consumers: warp (q, sub) owns the DMs q DQ + sub D + j of the block =====
+        const int q = warp & 3, sub = warp >> 2;
+        const uint32_t tq = tbase + ((uint32_t)(q * 32) << 16);
+        int ts = 0;
+        uint32_t tph = 0;
+        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+            const int blk = (int)(tile % a.nblk);
+            const long long rest = tile / a.nblk;
+            const int tt = (int)(rest % a.ntile_t), bb = (int)(rest / a.ntile_t);
+            const long long tile_t0 = (long long)tt * a.span;
+            const int nslab = a.nslab[blk];
+            float acc[D][P];
+#pragma unroll
+            for (int j = 0; j < D; ++j)
+#pragma unroll
+                for (int i = 0; i < P; ++i) acc[j][i] = 0.0f;
+#pragma unroll 1
+            for (int slab = 0; slab < nslab; ++slab) {
+                while (!mbar_try_wait(&tfull[ts * 4 + q], tph)) __nanosleep(64);      // no hot spinning beside the stager
+                tm_fence_after();
+                const uint32_t *te = tent + (ts * 4 + q) * TENT;
+                const int nq = (int)te[DQ * kTmQMax];
+                const uint32_t *ents = te + sub * D * kTmQMax;
+                const uint32_t tstage = tq + ts * kTmCols;
+#pragma unroll 1
+                for (int g = 0; g < nq; ++g) {
+                    uint32_t e[D];
+#pragma unroll
+                    for (int j = 0; j < D; ++j) e[j] = ents[j * kTmQMax + g];
+#pragma unroll
+                    for (int j = 0; j < D; ++j) {
+                        uint32_t v[16];
+                        tm_ld16(tstage + e[j], v);
+                        tm_wait_ld();
+#pragma unroll
+                        for (int i = 0; i < P; ++i) acc[j][i] += __uint_as_float(v[i]);
+                    }
+                }
+                tm_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tempty[ts * 4 + q]);
+                if (++ts == 2) { ts = 0; tph ^= 1; }
+            }
+            const int b = a.beam0 + bb;
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const int dl = q * DQ + sub * D + j, d = blk * DB + dl;
+                if (d >= a.ndms) continue;
+                const long long ts0 = tile_t0 - a.sigma[dl] + P * lane;
+                float *orow = a.out + ((size_t)b * a.ndms + d) * (size_t)a.nsamps;
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    const long long t = ts0 + i;
+                    if (t >= 0 && t < a.nsamps_out) orow[t] = acc[j][i];
+                }
+            }
+        }
+    }
+    tm_fence_before();
+    __syncthreads();
+    if (warp == kTmProducer) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
+}
+
 // ------------------------------------------------------------------ host side: the plan-time tables
 struct RowsGeom { int D, T, NW; };
 constexpr RowsGeom kGeomRowsF32 = {4, 16, 16};      // 64 DMs x 512 samples per tile
@@ -588,6 +847,149 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, const GroupRows &gr,
     return true;
 }
 
+// ---- tables of the TMEM variant (fp32): variable slabs of <= kTmQMax groups, packed so that every quadrant's rows fit a
+// TMEM stage of kTmCols columns and the block's rows fit the shared-memory stage.
+struct TmemGeom { int D, P; };
+constexpr TmemGeom kGeomTmem = {4, 15};            // 64 DMs x 480 samples per tile
+
+struct TmemHost {
+    std::vector<int4> rowdesc;
+    std::vector<uint32_t> tab;
+    std::vector<int32_t> nslab, sigma;
+};
+
+static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTables &tt, TmemHost &h)
+{
+    const int D = kGeomTmem.D, P = kGeomTmem.P, DQ = 4 * D, DB = 16 * D, span = 32 * P, al = 4;
+    const int nblk = (p->ndms + DB - 1) / DB, ng = gr.ngroups, G = gr.G;
+    const double f_lo = p->f_top + (p->nchans - 1) * p->foff;
+    const double smax = 4.148808e3 * p->dm_step * (1.0 / (f_lo * f_lo) - 1.0 / (p->f_top * p->f_top)) / p->tsamp;
+    h.sigma.resize(DB);
+    for (int dl = 0; dl < DB; ++dl) h.sigma[dl] = (int32_t)llround(0.5 * smax * dl);
+    auto dly = [&](int d, int c) { return (long long)p->h_delay[(size_t)d * p->nchans + c]; };
+    struct Use { int yrow; long long emin, emax; };
+    struct GroupUse { std::vector<Use> blk; std::vector<Use> quad[4]; int cols[4]; };
+    auto add_use = [](std::vector<Use> &u, int yr, long long e) {
+        auto it = std::find_if(u.begin(), u.end(), [&](const Use &x) { return x.yrow == yr; });
+        if (it == u.end()) u.push_back({yr, e, e});
+        else { it->emin = std::min(it->emin, e); it->emax = std::max(it->emax, e); }
+    };
+    const int tabw = 8 + 4 * kTmRQMax * 2 + DB * kTmQMax;
+    std::vector<std::vector<GroupUse>> gu(nblk, std::vector<GroupUse>(ng));
+    long long need_max = 0;
+    for (int blk = 0; blk < nblk; ++blk)
+        for (int gi = 0; gi < ng; ++gi) {
+            GroupUse &u = gu[blk][gi];
+            for (int dl = 0; dl < DB; ++dl) {
+                const int d = std::min(blk * DB + dl, p->ndms - 1), dle = d - blk * DB;     // DMs past the grid repeat the last one
+                const int yr = gr.yrow_of[(size_t)d * ng + gi];
+                const long long e = dly(d, gi * G) - h.sigma[dle];
+                add_use(u.blk, yr, e);
+                add_use(u.quad[dl / DQ], yr, e);
+            }
+            for (int q = 0; q < 4; ++q) {
+                u.cols[q] = 0;
+                for (const Use &x : u.quad[q]) u.cols[q] += (int)ceil_to(16 + (x.emax - x.emin), 8);   // the consumers load 16 columns
+                if (u.cols[q] > kTmCols || (int)u.quad[q].size() > kTmRQMax) return false;
+            }
+            if (u.blk.size() > 32) return false;
+            for (const Use &x : u.blk) need_max = std::max(need_max, x.emax - floor_to(x.emin, al) + span);
+        }
+    const int pitch = (int)ceil_to(need_max, al) + 16;       // + 16: the stagers read whole 8-column chunks of 16 + S columns
+    // greedy packing of consecutive groups into slabs
+    struct Slab { int g0, g1; };
+    std::vector<std::vector<Slab>> slabs(nblk);
+    int cs_max = 0, nslab_max = 0;
+    long long ngroups_total = 0, nslabs_total = 0;
+    double cols_total = 0;
+    for (int blk = 0; blk < nblk; ++blk) {
+        int g0 = 0;
+        while (g0 < ng) {
+            int rows = 0, cols[4] = {0, 0, 0, 0}, nrq[4] = {0, 0, 0, 0}, g1 = g0;
+            while (g1 < ng && g1 - g0 < kTmQMax) {
+                const GroupUse &u = gu[blk][g1];
+                bool fits = rows + (int)u.blk.size() <= 32;
+                for (int q = 0; q < 4; ++q) fits = fits && cols[q] + u.cols[q] <= kTmCols && nrq[q] + (int)u.quad[q].size() <= kTmRQMax;
+                if (!fits) break;
+                rows += (int)u.blk.size();
+                for (int q = 0; q < 4; ++q) { cols[q] += u.cols[q]; nrq[q] += (int)u.quad[q].size(); cols_total += u.cols[q]; }
+                ++g1;
+            }
+            if (g1 == g0) return false;
+            cs_max = std::max(cs_max, rows);
+            slabs[blk].push_back({g0, g1});
+            g0 = g1;
+        }
+        nslab_max = std::max(nslab_max, (int)slabs[blk].size());
+        ngroups_total += ng;
+        nslabs_total += (long long)slabs[blk].size();
+    }
+    const int CS = cs_max;
+    const size_t stage = (((size_t)CS * pitch * 4 + (size_t)tabw * 4) + 127) & ~(size_t)127;
+    const size_t fixed = (size_t)2 * 4 * (DQ * kTmQMax + 4) * 4 + 320;      // entry copies, barriers, TMEM base slot
+    const int stages = (int)std::min<size_t>(8, (kSmemBudget - fixed - 64) / stage);
+    if (stages < 2) return false;
+    h.rowdesc.assign((size_t)nblk * nslab_max * CS, make_int4(-1, 0, 0, 0));
+    h.tab.assign((size_t)nblk * nslab_max * tabw, 0u);
+    h.nslab.resize(nblk);
+    for (int blk = 0; blk < nblk; ++blk) {
+        h.nslab[blk] = (int32_t)slabs[blk].size();
+        for (size_t s = 0; s < slabs[blk].size(); ++s) {
+            int4 *rd = &h.rowdesc[((size_t)blk * nslab_max + s) * CS];
+            uint32_t *tab = &h.tab[((size_t)blk * nslab_max + s) * tabw];
+            int r = 0, nrq[4] = {0, 0, 0, 0}, tcol[4] = {0, 0, 0, 0};
+            tab[4] = (uint32_t)(slabs[blk][s].g1 - slabs[blk][s].g0);
+            for (int gi = slabs[blk][s].g0; gi < slabs[blk][s].g1; ++gi) {
+                const GroupUse &u = gu[blk][gi];
+                const int qi = gi - slabs[blk][s].g0;
+                for (size_t k = 0; k < u.blk.size(); ++k) {
+                    const long long rs = floor_to(u.blk[k].emin, al);
+                    rd[r + k] = make_int4(u.blk[k].yrow, (int)rs, (int)ceil_to(u.blk[k].emax - rs + span, al), 0);
+                }
+                for (int q = 0; q < 4; ++q) {
+                    std::vector<int> col_of(u.quad[q].size());
+                    for (size_t k = 0; k < u.quad[q].size(); ++k) {
+                        const Use &x = u.quad[q][k];
+                        size_t kb = 0;
+                        while (u.blk[kb].yrow != x.yrow) ++kb;
+                        const long long rs = floor_to(u.blk[kb].emin, al);
+                        const int n8 = (int)ceil_to(16 + (x.emax - x.emin), 8) / 8;
+                        const int slot = nrq[q]++;
+                        tab[8 + (q * kTmRQMax + slot) * 2] = (uint32_t)((long long)(r + kb) * pitch + (x.emin - rs));
+                        tab[8 + (q * kTmRQMax + slot) * 2 + 1] = (uint32_t)tcol[q] | ((uint32_t)n8 << 16);
+                        col_of[k] = tcol[q];
+                        tcol[q] += 8 * n8;
+                    }
+                    for (int dq = 0; dq < DQ; ++dq) {
+                        const int dl = q * DQ + dq;
+                        const int d = std::min(blk * DB + dl, p->ndms - 1), dle = d - blk * DB;
+                        const int yr = gr.yrow_of[(size_t)d * ng + gi];
+                        size_t k = 0;
+                        while (u.quad[q][k].yrow != yr) ++k;
+                        const long long e = dly(d, gi * G) - h.sigma[dle];
+                        tab[8 + 4 * kTmRQMax * 2 + (size_t)dl * kTmQMax + qi] = (uint32_t)(col_of[k] + (e - u.quad[q][k].emin));
+                    }
+                }
+                r += (int)u.blk.size();
+            }
+            for (int q = 0; q < 4; ++q) tab[q] = (uint32_t)nrq[q];
+        }
+    }
+    tt.D = D; tt.P = P; tt.DB = DB; tt.span = span; tt.CS = CS; tt.pitch = pitch; tt.stages = stages;
+    tt.nslab_max = nslab_max; tt.nblk = nblk; tt.tabw = tabw;
+    tt.sigma_max = *std::max_element(h.sigma.begin(), h.sigma.end());
+    tt.smem_bytes = (size_t)stages * stage + fixed;
+    tt.groups_per_slab = (double)ngroups_total / (double)nslabs_total;
+    tt.cols_per_group = cols_total / (4.0 * (double)ngroups_total);
+    return true;
+}
+
+static void free_tmem_tables(TmemTables *tt)
+{
+    cudaFree(tt->d_rowdesc); cudaFree(tt->d_tab); cudaFree(tt->d_nslab); cudaFree(tt->d_sigma);
+    *tt = TmemTables();
+}
+
 static void free_rows_tables(RowsTables *rt)
 {
     cudaFree(rt->d_rowdesc); cudaFree(rt->d_ent); cudaFree(rt->d_sigma); cudaFree(rt->d_group_row0); cudaFree(rt->d_ydelta);
@@ -602,6 +1004,7 @@ static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &can
 {
     RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
     free_rows_tables(&rt);
+    if (f32) free_tmem_tables(&p->tmem_f32);
     const RowsGeom geom = f32 ? kGeomRowsF32 : kGeomRowsU16;
     // candidates in the order of their modelled cost; the first whose tables fit the kernel's limits is taken
     std::vector<const GroupRows *> order;
@@ -617,6 +1020,21 @@ static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &can
             return MDSM_ECUDA;
         }
         rt.ok = true;
+        if (f32) {
+            // the TMEM variant of the main kernel shares the pre-pass, the scratch layout and the group size
+            free_tmem_tables(&p->tmem_f32);
+            TmemHost th;
+            TmemTables &tt = p->tmem_f32;
+            if (build_tmem_tables(p, *gr, tt, th)) {
+                if (!upload((int4 **)&tt.d_rowdesc, th.rowdesc) || !upload(&tt.d_tab, th.tab) || !upload(&tt.d_nslab, th.nslab) ||
+                    !upload(&tt.d_sigma, th.sigma)) {
+                    mdsm_set_error("dedispersion table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+                    free_tmem_tables(&tt);
+                    return MDSM_ECUDA;
+                }
+                tt.ok = true;
+            }
+        }
         return MDSM_OK;
     }
     return MDSM_OK;                                                    // no table: the direct kernel runs
@@ -655,6 +1073,7 @@ int mdsm_rows_build_tables(mdsm_plan *p)
 
 void mdsm_rows_free_tables(mdsm_plan *p)
 {
+    free_tmem_tables(&p->tmem_f32);
     free_rows_tables(&p->rows_f32);
     free_rows_tables(&p->rows_u8);
 }
@@ -708,6 +1127,23 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
         MDSM_CUDA_TRY(cudaGetLastError());
         p->launches += 1;
 
+        int rc;
+        const TmemTables &tt = p->tmem_f32;
+        if (f32 && tt.ok && p->dedisp_kernel == 3) {          // experimental variant: only on request
+            TmemArgs a;
+            a.y = (const float *)scratch; a.out = (float *)d_out;
+            a.rowdesc = (const int4 *)tt.d_rowdesc; a.tab = tt.d_tab; a.nslab = tt.d_nslab; a.sigma = tt.d_sigma;
+            a.beam0 = bs; a.nslots = nslots; a.nyrows = rt.nyrows; a.ndms = p->ndms;
+            a.nblk = tt.nblk; a.ntile_t = (int)((p->nsamps_out + tt.sigma_max + tt.span - 1) / tt.span);
+            a.nslab_max = tt.nslab_max; a.CS = tt.CS; a.pitch = tt.pitch; a.stages = tt.stages; a.tabw = tt.tabw; a.span = tt.span;
+            a.ntiles = (long long)tt.nblk * a.ntile_t * n;
+            a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out; a.ystride = rt.ystride;
+            auto kern = dedisperse_tmem_kernel<kGeomTmem.D, kGeomTmem.P>;
+            MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tt.smem_bytes));
+            kern<<<(int)std::min<long long>(a.ntiles, p->sm_count), kTmWarps * 32, tt.smem_bytes, st>>>(a);
+            MDSM_CUDA_TRY(cudaGetLastError());
+            rc = MDSM_OK;
+        } else {
         RowsArgs a;
         a.y = scratch; a.out = d_out;
         a.rowdesc = (const int4 *)rt.d_rowdesc; a.ent = rt.d_ent; a.sigma = rt.d_sigma;
@@ -717,9 +1153,9 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
         a.ntiles = (long long)rt.nblk * ntile_t * n;
         a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out; a.ystride = rt.ystride;
         const int grid_main = (int)std::min<long long>(a.ntiles, p->sm_count);
-        int rc;
         if (f32) rc = launch_rows<RowsTraits<kGeomRowsF32.D, kGeomRowsF32.T, kGeomRowsF32.NW, true>>(a, rt.smem_bytes, grid_main, st);
         else rc = launch_rows<RowsTraits<kGeomRowsU16.D, kGeomRowsU16.T, kGeomRowsU16.NW, false>>(a, rt.smem_bytes, grid_main, st);
+        }
         if (rc != MDSM_OK) return rc;
         p->launches += 1;
     }

@@ -46,6 +46,22 @@ struct RowsTables {
     int16_t *d_ydelta = nullptr;                  // [nyrows][8]
 };
 
+// Tables of the TMEM-window variant of the main kernel (fp32; dedisperse_rows.cu): the same
+// pre-summed rows, staged TMA -> shared memory -> tensor memory, consumed with tcgen05.ld at run-time column offsets.
+struct TmemTables {
+    bool ok = false;
+    int D = 0, P = 0, DB = 0, span = 0;           // DMs per warp, outputs per lane and DM, DMs per block, outputs per tile and DM
+    int CS = 0, pitch = 0, stages = 0;            // row slots per shared-memory stage, words per slot, stages
+    int nslab_max = 0, nblk = 0, tabw = 0;        // slabs per block (padded), DM blocks, 32-bit words of a slab's table slice
+    int sigma_max = 0;
+    size_t smem_bytes = 0;
+    double groups_per_slab = 0.0, cols_per_group = 0.0;   // statistics for kernel_info
+    void *d_rowdesc = nullptr;                    // int4 [nblk][nslab_max][CS]
+    uint32_t *d_tab = nullptr;                    // [nblk][nslab_max][tabw]
+    int32_t *d_nslab = nullptr;                   // [nblk]
+    int32_t *d_sigma = nullptr;                   // [DB]
+};
+
 struct mdsm_plan {
     int nbeams, nchans, ndms;
     double f_top, foff, tsamp, dm_low, dm_step;
@@ -67,6 +83,7 @@ struct mdsm_plan {
     int dedisp_kernel = 0;            // option "dedisp_kernel": 0 auto, 1 direct, 2 rows
     int group_size = 0;               // option "group_size": channels per pre-summed group, 0 = chosen by the cost model
     RowsTables rows_f32, rows_u8;
+    TmemTables tmem_f32;
     void *d_scratch_f32 = nullptr, *d_scratch_u8 = nullptr;     // pre-summed rows [slots][nyrows][ystride] (mdsm_plan_reserve)
     int scratch_slots_f32 = 0, scratch_slots_u8 = 0;            // beams the scratch holds at a time
     size_t scratch_bytes_f32 = 0, scratch_bytes_u8 = 0;

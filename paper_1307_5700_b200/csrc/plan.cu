@@ -166,7 +166,7 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
 {
     MDSM_REQUIRE(p && key, "null argument");
     if (strcmp(key, "dedisp_kernel") == 0) {
-        MDSM_REQUIRE(value >= 0 && value <= 2, "dedisp_kernel must be 0 (auto), 1 (direct) or 2 (pre-summed rows)");
+        MDSM_REQUIRE(value >= 0 && value <= 3, "dedisp_kernel must be 0 (auto), 1 (direct), 2 (pre-summed rows, shared-memory operands) or 3 (pre-summed rows, TMEM operands)");
         p->dedisp_kernel = (int)value;
         return MDSM_OK;
     }
@@ -226,6 +226,7 @@ extern "C" int mdsm_dedisperse(mdsm_plan *p, const void *d_in, int dtype, int be
     if (p->dedisp_kernel == 1 || (p->dedisp_kernel == 0 && !rt.ok))
         return mdsm_launch_dedisperse_direct(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
     MDSM_REQUIRE(rt.ok, "the pre-summed-rows kernel has no tables for this plan (see mdsm_plan_kernel_info)");
+    MDSM_REQUIRE(p->dedisp_kernel != 3 || (dtype == MDSM_F32 && p->tmem_f32.ok), "the TMEM variant has no tables for this plan / dtype");
     MDSM_REQUIRE(dtype == MDSM_F32 ? p->d_scratch_f32 != nullptr : p->d_scratch_u8 != nullptr,
                  "dedispersion scratch not reserved: call mdsm_plan_reserve(plan, dtype, 0) once before mdsm_dedisperse");
     return mdsm_launch_dedisperse_rows(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
@@ -280,8 +281,17 @@ extern "C" int mdsm_plan_kernel_info(const mdsm_plan *p, int dtype, char *buf, i
         snprintf(buf, (size_t)buflen, "kernel=direct reason=%s", p->dedisp_kernel == 1 ? "option" : "no_tables");
         return 0;
     }
+    const bool tmem = f32 && p->tmem_f32.ok && p->dedisp_kernel == 3;
+    const TmemTables &tt = p->tmem_f32;
+    if (tmem)
+        snprintf(buf, (size_t)buflen,
+                 "kernel=rows operands=tmem group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%.2f tmem_cols_per_group=%.1f "
+                 "row_slots=%d row_pitch=%d stages=%d smem_bytes=%zu nyrows=%d scratch_slots=%d scratch_bytes=%zu",
+                 rt.G, tt.DB, tt.span, tt.groups_per_slab, tt.cols_per_group, tt.CS, tt.pitch, tt.stages, tt.smem_bytes, rt.nyrows,
+                 p->scratch_slots_f32, p->scratch_bytes_f32);
+    else
     snprintf(buf, (size_t)buflen,
-             "kernel=rows group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%d row_slots=%d row_pitch=%d stages=%d "
+             "kernel=rows operands=smem group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%d row_slots=%d row_pitch=%d stages=%d "
              "smem_bytes=%zu nyrows=%d rows_per_block=%.0f scratch_slots=%d scratch_bytes=%zu",
              rt.G, rt.DB, rt.stride, rt.Q, rt.CS, rt.pitch, rt.stages, rt.smem_bytes, rt.nyrows, rt.rows_per_block,
              f32 ? p->scratch_slots_f32 : p->scratch_slots_u8, f32 ? p->scratch_bytes_f32 : p->scratch_bytes_u8);

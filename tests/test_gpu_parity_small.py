@@ -283,3 +283,23 @@ def test_add_peak_microbenchmark_runs():
     for kind in (0, 1, 2):
         v = m.mdsm_measure_add_peak(kind)
         assert 1e13 < v < 1e14
+
+
+@pytest.mark.parametrize("name", ["cfg1", "ragged", "multi_tile", "wide", "parts"])
+def test_tmem_operand_variant_matches_the_oracle(name):
+    """dedisp_kernel = 3: the same pre-summed rows with the operand windows staged in tensor memory (tcgen05.st /
+    tcgen05.ld at run-time column offsets).  Experimental (slower than the shared-memory variant), kept parity-green."""
+    torch = _torch()
+    args = SHAPES[name]
+    nb, nc, ns = args[0], args[1], args[5]
+    x = generate(CONFIGS[1]) if name == "cfg1" else _rand_input((nb, nc, ns), np.float32, 43)
+    d = oracle.delay_table(args[1], args[2], args[3], args[4], args[6], args[7], args[8])
+    ref, ab = oracle.dedisperse(x, d)
+    with Plan(args) as p:
+        p.set_option("dedisp_kernel", 3)
+        info = p.info(p.m.MDSM_F32)
+        if info.get("operands") != "tmem":
+            pytest.skip(f"no TMEM tables for this plan: {info}")
+        out = p.dedisperse(torch.from_numpy(x).cuda(), kernel=3)
+        assert_f32_parity(out_to_numpy(out, p.nsamps_out), ref, ab, name)
+        assert np.all(out[:, :, p.nsamps_out:].cpu().numpy() == -7)

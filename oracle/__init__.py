@@ -19,6 +19,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mdsm_oracle.c")
+_SRC_NEXT = os.path.join(_HERE, "mdsm_oracle_next.c")          # the SURVEY 8(f) rows
 _LIB = os.path.join(_HERE, "libmdsm_oracle.so")
 # -ffp-contract=off / no fast-math: every fp64 op is a single IEEE op in the order written.
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-Wall"]
@@ -28,8 +29,8 @@ EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr"
 
 def build(force: bool = False) -> str:
     """Compile the C oracle with gcc if the .so is missing or older than the source."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.run(["gcc", *CFLAGS, "-o", _LIB, _SRC, "-lm"], check=True)
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_NEXT)):
+        subprocess.run(["gcc", *CFLAGS, "-o", _LIB, _SRC, _SRC_NEXT, "-lm"], check=True)
     return _LIB
 
 
@@ -44,6 +45,10 @@ def _L():
         _lib.orc_detect_f64.restype = c_int64
         _lib.orc_detect_u32.restype = c_int64
         _lib.orc_num_threads.restype = c_int
+        _lib.orc_dbscan.restype = c_int64
+        _lib.orc_fdbscan.restype = c_int64
+        _lib.orc_dm_response.restype = c_double
+        _lib.orc_zeta.restype = c_double
     return _lib
 
 
@@ -199,3 +204,110 @@ def mulaw_u8(x: np.ndarray, mu: float):
     xmax = np.zeros(1, dtype=np.float32)
     _L().orc_mulaw_u8(_p(x), c_int64(x.size), c_double(mu), _p(code), _p(xmax))
     return code, float(xmax[0])
+
+
+# ---------------------------------------------------------------- SURVEY 8(f) rows (mdsm_oracle_next.c)
+def polyfit_u(y: np.ndarray, order: int) -> np.ndarray:
+    """Least-squares coefficients (ascending powers of u = 2c/(n-1) - 1) of an order-p polynomial through y[c]."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    coef = np.zeros(order + 1, dtype=np.float64)
+    rc = _L().orc_polyfit_u(_p(y), c_int(y.size), c_int(order), _p(coef))
+    if rc != 0:
+        raise ValueError("singular fit")
+    return coef
+
+
+def bandpass_clip(x: np.ndarray, window: int, order: int, k_mask: float, k_chan: float, k_spec: float, subtract: bool):
+    """The paper's bandpass-fit RFI stage (readings H-*), in place on x [nb][nchans][nsamps] float32.
+    Returns dict(chan_mask, spec_mask, fit, bpi, rmse, mean_bp, std_bp, nmasked)."""
+    assert x.dtype == np.float32 and x.ndim == 3 and x.flags.c_contiguous
+    nb, nc, ns = x.shape
+    cm = np.zeros((nb, nc, ns // window), dtype=np.uint8)
+    sm = np.zeros((nb, ns), dtype=np.uint8)
+    fit = np.zeros((nb, nc), dtype=np.float64)
+    bpi = np.zeros((nb, nc), dtype=np.float64)
+    st = np.zeros((nb, 4), dtype=np.float64)
+    rc = _L().orc_bandpass_clip_f32(_p(x), c_int(nb), c_int(nc), c_int64(ns), c_int(window), c_int(order), c_double(k_mask),
+                                    c_double(k_chan), c_double(k_spec), c_int(1 if subtract else 0), _p(cm), _p(sm), _p(fit),
+                                    _p(bpi), _p(st))
+    if rc != 0:
+        raise ValueError(f"orc_bandpass_clip_f32 returned {rc}")
+    return {"chan_mask": cm, "spec_mask": sm, "fit": fit, "bpi": bpi, "rmse": st[:, 0].copy(), "mean_bp": st[:, 1].copy(),
+            "std_bp": st[:, 2].copy(), "nmasked": st[:, 3].astype(np.int64)}
+
+
+def _points(pts):
+    pts = np.ascontiguousarray(pts, dtype=np.float64)
+    assert pts.ndim == 2 and pts.shape[1] == 3
+    return pts
+
+
+def dbscan(pts, eps, min_pts: int):
+    """Textbook DBSCAN with a per-dimension box neighbourhood. Returns (labels int32, nclusters)."""
+    pts = _points(pts)
+    eps = np.ascontiguousarray(eps, dtype=np.float64)
+    lab = np.empty(pts.shape[0], dtype=np.int32)
+    n = _L().orc_dbscan(_p(pts), c_int64(pts.shape[0]), _p(eps), c_int(min_pts), _p(lab))
+    return lab, int(n)
+
+
+def fdbscan(pts, eps, min_pts: int):
+    """FDBSCAN (representative seeds; reading K-ii). Returns (labels, nclusters, region queries made)."""
+    pts = _points(pts)
+    eps = np.ascontiguousarray(eps, dtype=np.float64)
+    lab = np.empty(pts.shape[0], dtype=np.int32)
+    nq = np.zeros(1, dtype=np.int64)
+    n = _L().orc_fdbscan(_p(pts), c_int64(pts.shape[0]), _p(eps), c_int(min_pts), _p(lab), _p(nq))
+    return lab, int(n), int(nq[0])
+
+
+def dm_response(zeta: float) -> float:
+    """Eq. 3 (PAPER.md:136)."""
+    return float(_L().orc_dm_response(c_double(zeta)))
+
+
+def zeta(ddm: float, bw_mhz: float, w_ms: float, nu_ghz: float) -> float:
+    """Eq. 4 (PAPER.md:140)."""
+    return float(_L().orc_zeta(c_double(ddm), c_double(bw_mhz), c_double(w_ms), c_double(nu_ghz)))
+
+
+def classify_cluster(t, dm_idx, snr, dm_low, dm_step, tsamp, bw_mhz, nu_ghz, k_smooth, rmse_max):
+    """The 8-step classifier of PAPER.md:144-156 for one cluster. Returns dict(cls, dm_idx, snr, width_ms, rmse)."""
+    t = np.ascontiguousarray(t, dtype=np.int32)
+    d = np.ascontiguousarray(dm_idx, dtype=np.int32)
+    s = np.ascontiguousarray(snr, dtype=np.float32)
+    res = np.zeros(5, dtype=np.float64)
+    rc = _L().orc_classify_cluster(_p(t), _p(d), _p(s), c_int64(t.size), c_double(dm_low), c_double(dm_step), c_double(tsamp),
+                                   c_double(bw_mhz), c_double(nu_ghz), c_int(k_smooth), c_double(rmse_max), _p(res))
+    if rc != 0:
+        raise ValueError("bad arguments")
+    return {"cls": int(res[0]), "dm_idx": int(res[1]), "snr": float(res[2]), "width_ms": float(res[3]), "rmse": float(res[4])}
+
+
+def mulaw_c4(volt: np.ndarray, mu: float):
+    """2 x 16 bit -> 2 x 4 bit mu-law codes packed into one byte (Eq. 5; reading G-ii). Returns (bytes, xmax)."""
+    assert volt.dtype == np.int16 and volt.shape[-1] == 2 and volt.flags.c_contiguous and mu > 0
+    out = np.empty(volt.shape[:-1], dtype=np.uint8)
+    xmax = np.zeros(1, dtype=np.int32)
+    _L().orc_mulaw_c4(_p(volt), c_int64(out.size), c_double(mu), _p(out), _p(xmax))
+    return out, int(xmax[0])
+
+
+def dedisperse_u16(x: np.ndarray, delay: np.ndarray) -> np.ndarray:
+    """Brute-force dedispersion of uint16 samples [nb][nchans][nsamps] -> uint32 [nb][ndms][nsamps_out] (exact)."""
+    assert x.dtype == np.uint16 and x.ndim == 3 and x.flags.c_contiguous
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    nb, nc, ns = x.shape
+    nso = ns - int(delay.max())
+    out = np.empty((nb, delay.shape[0], nso), dtype=np.uint32)
+    _L().orc_dedisperse_u16_rows(_p(x), c_int(nb), c_int(nc), c_int64(ns), _p(delay), c_int(delay.shape[0]), c_int64(nso), _p(out))
+    return out
+
+
+def unpack_u4(x: np.ndarray) -> np.ndarray:
+    """4-bit samples, two per byte along time (low nibble first) [..., nsamps/2] uint8 -> [..., nsamps] uint16."""
+    assert x.dtype == np.uint8
+    out = np.empty(x.shape[:-1] + (x.shape[-1] * 2,), dtype=np.uint16)
+    out[..., 0::2] = x & 15
+    out[..., 1::2] = x >> 4
+    return out

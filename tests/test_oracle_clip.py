@@ -166,3 +166,32 @@ def test_u8_threshold_arithmetic_by_hand():
     assert abs(r["chan_thr"][0, 0] - (40 + 2 * math.sqrt(300) * math.sqrt(2))) < 1e-12
     assert x[0, 0].tolist() == [10, 10, 10, 10, 20, 20, 20, 20]     # repl = (160+4)//8 = 20
     assert r["repl"][0].tolist() == [20.0, 20.0]
+
+
+def test_channel_threshold_tie_is_not_a_flag_strict_greater():
+    """Reading B-v / PAPER.md:79 "exceeds": a chunk sum EQUAL to the threshold is not flagged.  Worked by hand:
+    x = 0,0,0,0,4,4,4,4: mean 2, Q/N = 8, var 4, sig 2; W = 4: thr = 4*2 + k*2*sqrt(4) = 8 + 4k; chunk sums 0, 16."""
+    def run(k):
+        x = np.array([[[0, 0, 0, 0, 4, 4, 4, 4]]], dtype=np.uint8)
+        r = oracle.rfi_clip(x, 4, k, 1e9, debug=True)
+        return r, x
+    r, x = run(2.0)                                            # thr = 16 = the second chunk's sum
+    assert r["chan_thr"][0, 0] == 16.0 and not r["chan_mask"].any() and x[0, 0].tolist() == [0, 0, 0, 0, 4, 4, 4, 4]
+    r, x = run(1.9999)                                         # just below: flagged, its neighbour by dilation, both replaced by 2
+    assert r["chan_mask"][0, 0].tolist() == [1, 1] and x[0, 0].tolist() == [2] * 8
+
+
+def test_spectrum_threshold_by_hand_and_its_tie():
+    """B3 worked by hand: two channels 0,2 -> spectrum sums s = 0, 4: mean_s 2, M2/N = 8, var 4, sig 2;
+    thr = 2 + 2 k_spec.  k_spec = 1 -> thr = 4 = s_1: not flagged (strict); k_spec = 0.999 -> flagged and replaced by
+    repl_c = (2 + 1) // 2 = 1."""
+    def run(k):
+        x = np.array([[[0, 2], [0, 2]]], dtype=np.uint8)
+        r = oracle.rfi_clip(x, 1, 1e9, k, debug=True)
+        return r, x
+    r, x = run(1.0)
+    assert r["spec_thr"][0].tolist() == [4.0, 2.0, 2.0]
+    assert not r["spec_mask"].any() and x[0].tolist() == [[0, 2], [0, 2]]
+    r, x = run(0.999)
+    assert r["spec_mask"][0].tolist() == [0, 1] and x[0].tolist() == [[0, 1], [0, 1]]
+    assert abs(r["spec_thr"][0, 0] - 3.998) < 1e-12

@@ -55,4 +55,5 @@ def test_detrend_exact_line_and_constant_give_zeros():
     x = np.stack([2.0 + 0.5 * t, np.full(n, 7.0, dtype=np.float32)]).astype(np.float32)
     y, p = oracle.detrend(x, n)
     assert p[0, 1] == pytest.approx(0.5) and p[1, 1] == 0.0 and p[1, 2] == 0.0
-    assert np.all(y[1] == 0.0) and np.all(np.abs(y[0]) < 1e-3) or p[0, 2] < 1e-12
+    # an exact line leaves a zero residual: both series become zeros (reading E-ii)
+    assert p[0, 2] < 1e-6 and np.all(y[0] == 0.0) and np.all(y[1] == 0.0)

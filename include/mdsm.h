@@ -105,6 +105,27 @@ int mdsm_rfi_clip(mdsm_plan *plan, void *d_in, int dtype, int beam0, int nb,
                   int window, double k_chan, double k_spec,
                   uint8_t *d_chan_mask, uint8_t *d_spec_mask, void *cuda_stream);
 
+/* The paper's own RFI stage (Fig. 3; readings H-i..H-vii of DESIGN.md section 3) as an
+ * alternative to mdsm_rfi_clip, for float power data, in place, per beam:
+ *  1. averaged bandpass bp[c] = mean_t x[c][t];
+ *  2. channels with (bp[c] - median bp) > k_mask * 1.4826 * MAD are masked and replaced by the mean of the nearest
+ *     un-masked channel on either side ("interpolating the bandpass");
+ *  3. least-squares polynomial of order `order` (<= 12, < nchans) through the interpolated bandpass -> fit[c]; rmse of the
+ *     fit; mean_bp, std_bp = mean and population standard deviation of the interpolated bandpass over the channels;
+ *  4. channel thresholding: chunks of `window` samples whose MEAN > fit[c] + k_chan * rmse are flagged together with their
+ *     two time neighbours and overwritten with (float)fit[c];
+ *  5. spectrum thresholding on the modified data: spectra whose mean over the channels > mean_bp + k_spec * std_bp are
+ *     overwritten with (float)fit[c];
+ *  6. subtract != 0: (float)fit[c] is subtracted from every sample (flagged samples become exactly 0).
+ * The fit runs on the GPU (one CTA per beam), so the call is asynchronous like the other stage calls and allocates nothing.
+ * d_chan_mask [nbeams][nchans][nsamps/window], d_spec_mask [nbeams][nsamps] (0/1; either may be NULL);
+ * d_fit (may be NULL) [nbeams][nchans][2] doubles = fit, interpolated bandpass; d_stats (may be NULL) [nbeams][4] doubles =
+ * rmse, mean_bp, std_bp, number of masked channels.  MDSM_EINVAL: bad beam range / window / order, nchans too large for
+ * the shared-memory sort (> 8192). */
+int mdsm_bandpass_clip(mdsm_plan *plan, float *d_in, int beam0, int nb, int window, int order, double k_mask,
+                       double k_chan, double k_spec, int subtract, uint8_t *d_chan_mask, uint8_t *d_spec_mask,
+                       double *d_fit, double *d_stats, void *cuda_stream);
+
 /* Brute-force incoherent dedispersion:
  *   out[b][d][t] = sum_c in[b][c][t + delay(d,c)],   t in [0, nsamps_out)
  * MDSM_F32: float in, float out (fp32 accumulation; |err| <= 1e-5 * sum_c|in| + 1e-6).

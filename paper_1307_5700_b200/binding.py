@@ -18,7 +18,7 @@ __all__ = [
     "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
     "mdsm_plan_reserve", "mdsm_plan_kernel_info",
-    "mdsm_rfi_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
+    "mdsm_rfi_clip", "mdsm_bandpass_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
 ]
 
 MDSM_F32, MDSM_U8 = 0, 1
@@ -68,6 +68,9 @@ def _load():
     L.mdsm_rfi_clip.restype = c_int
     L.mdsm_rfi_clip.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_double, c_double, c_void_p,
                                 c_void_p, c_void_p]
+    L.mdsm_bandpass_clip.restype = c_int
+    L.mdsm_bandpass_clip.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_double, c_double, c_double, c_int,
+                                     c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     L.mdsm_dedisperse.restype = c_int
     L.mdsm_dedisperse.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
     L.mdsm_detect.restype = c_int
@@ -191,6 +194,12 @@ def mdsm_rfi_clip(plan, d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask=Non
                   stream=None, dtype=None) -> None:
     _check(_L.mdsm_rfi_clip(plan, _ptr(d_in), _dtype_of(d_in, dtype), beam0, nb, window, k_chan, k_spec,
                             _ptr(d_chan_mask), _ptr(d_spec_mask), _stream(stream)))
+
+
+def mdsm_bandpass_clip(plan, d_in, beam0, nb, window, order, k_mask, k_chan, k_spec, subtract, d_chan_mask=None,
+                       d_spec_mask=None, d_fit=None, d_stats=None, stream=None) -> None:
+    _check(_L.mdsm_bandpass_clip(plan, _ptr(d_in), beam0, nb, window, order, k_mask, k_chan, k_spec, int(bool(subtract)),
+                                 _ptr(d_chan_mask), _ptr(d_spec_mask), _ptr(d_fit), _ptr(d_stats), _stream(stream)))
 
 
 def mdsm_dedisperse(plan, d_in, beam0, nb, d_out, stream=None, dtype=None) -> None:

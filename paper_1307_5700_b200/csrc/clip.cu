@@ -82,7 +82,9 @@ template <typename A> __device__ A block_sum(A v, A *red /*[kWarps]*/)
 // mode 0: chunk = g lanes of one warp iteration (g power of two <= 32)
 // mode 1: chunk = g/32 warp iterations of one warp (g % 32 == 0)
 // mode 2: generic scalar path (any window, any alignment); chunk sums are recomputed from global
-template <typename T, int MODE>
+// STAGE 0: north_star's clip (statistics of the row itself); STAGE 1: the paper's bandpass stage (threshold on the chunk
+// MEAN and replacement value come from the fit, chan_stats[b][c] = fit, threshold, -, (float)fit)
+template <typename T, int MODE, int STAGE = 0>
 __global__ void __launch_bounds__(kThreads)
 clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps, int window, double k_chan,
                     double *__restrict__ chan_stats, uint8_t *__restrict__ chan_mask)
@@ -142,6 +144,13 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
     S = block_sum(S, red);
     Q = block_sum(Q, red);
 
+    double thr_fit = 0.0;
+    T repl_fit = 0;
+    if (STAGE == 1) {
+        const double *st = chan_stats + ((size_t)b * nchans + c) * 4;
+        thr_fit = st[1];
+        repl_fit = (T)st[3];
+    }
     // B1: per-channel statistics, single IEEE ops in the oracle's order
     const double dN = (double)nsamps;
     const double mean = __ddiv_rn((double)S, dN);
@@ -154,10 +163,11 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
         repl = (T)(((unsigned long long)S + (unsigned long long)(nsamps / 2)) / (unsigned long long)nsamps);
     else
         repl = (T)mean;
-    if (tid == 0) {
+    if (STAGE == 0 && tid == 0) {
         double *st = chan_stats + ((size_t)b * nchans + c) * 4;
         st[0] = mean; st[1] = sig; st[2] = thr; st[3] = (double)repl;
     }
+    if (STAGE == 1) repl = repl_fit;
 
     // B2: raw flags
     for (long long j = tid; j < nchunk; j += kThreads) {
@@ -169,7 +179,7 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
             for (int k = 0; k < window; ++k) s += (Acc)row[j * window + k];
             C = (double)s;
         }
-        raw[j] = (C > thr) ? 1 : 0;
+        raw[j] = (STAGE == 1 ? (__ddiv_rn(C, (double)window) > thr_fit) : (C > thr)) ? 1 : 0;
     }
     __syncthreads();
     // dilation by one chunk in time, mask output, in-place replacement
@@ -305,6 +315,213 @@ clip_spec_apply_kernel(T *__restrict__ in, int beam0, int nchans, long long nsam
     }
 }
 
+// ------------------------------------------------------------------ the paper's bandpass-fit stage
+// PAPER.md:71-81, readings H-i..H-vii of DESIGN.md section 3; the oracle is orc_bandpass_clip_f32.  The paper fits the
+// bandpass on the CPU between two kernels ("copied back to CPU memory"); here the fit is one small CTA
+// per beam, so the whole stage stays asynchronous on the caller's stream:
+//   bp_rowmean_kernel   H1: averaged bandpass bp[c] (one CTA per row, fp64)
+//   bp_fit_kernel       H2-H4: median/MAD masking (bitonic sort in shared memory), neighbour interpolation, order-p
+//                       normal equations (block reductions) solved by one thread, fit, rmse, mean/std of the bandpass
+//   clip_channel_kernel<float, MODE, 1>   H5 with the fitted thresholds and replacement values
+//   clip_spec_sum_kernel                  column sums of the modified data
+//   bp_spec_apply_kernel  H6 + H7: spectrum flags, fitted-value replacement, bandpass subtraction
+__global__ void __launch_bounds__(kThreads)
+bp_rowmean_kernel(const float *__restrict__ in, int beam0, int nchans, long long nsamps, int vec, double *__restrict__ bp)
+{
+    __shared__ double red[kWarps];
+    const int c = blockIdx.x, b = beam0 + blockIdx.y;
+    const float *row = in + ((size_t)b * nchans + c) * (size_t)nsamps;
+    double S = 0.0;
+    if (vec) {
+        const float4 *v = reinterpret_cast<const float4 *>(row);
+        for (long long i = threadIdx.x; i < nsamps / 4; i += kThreads) {
+            const float4 x = v[i];
+            S += ((double)x.x + (double)x.y) + ((double)x.z + (double)x.w);
+        }
+    } else {
+        for (long long t = threadIdx.x; t < nsamps; t += kThreads) S += (double)row[t];
+    }
+    S = block_sum(S, red);
+    if (threadIdx.x == 0) bp[(size_t)b * nchans + c] = __ddiv_rn(S, (double)nsamps);
+}
+
+constexpr int kFitThreads = 1024;
+constexpr int kFitMaxOrder = 12;
+
+__device__ void bitonic_sort(double *a, int n /* power of two */)
+{
+    for (int k = 2; k <= n; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const double x = a[i], y = a[l];
+                    const bool up = (i & k) == 0;
+                    if ((x > y) == up) { a[i] = y; a[l] = x; }
+                }
+            }
+        }
+    __syncthreads();
+}
+
+__device__ double fit_block_sum(double v, double *red /*[32]*/)
+{
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += red[i];
+    return t;
+}
+
+// chan_stats[b][c][4] = fit, fit + k_chan*rmse (threshold on the chunk MEAN), interpolated bandpass, (double)(float)fit
+// spec_stats[b][4]    = mean_bp + k_spec*std_bp, rmse, mean_bp, std_bp;  out_stats[b][4] = rmse, mean_bp, std_bp, masked channels
+__global__ void __launch_bounds__(kFitThreads)
+bp_fit_kernel(const double *__restrict__ bp_all, int beam0, int nchans, int npad, int order, double k_mask, double k_chan,
+              double k_spec, double *__restrict__ chan_stats, double *__restrict__ spec_stats, double *__restrict__ out_fit,
+              double *__restrict__ out_stats)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *bp = reinterpret_cast<double *>(smem_raw);          // [nchans]
+    double *srt = bp + nchans;                                  // [npad]
+    double *bpi = srt + npad;                                   // [nchans]
+    __shared__ double red[32];
+    __shared__ double coef[kFitMaxOrder + 1];
+    __shared__ double sums[3 * kFitMaxOrder + 2];
+    __shared__ int s_nmask;
+    const int b = beam0 + blockIdx.x, tid = threadIdx.x;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    for (int c = tid; c < npad; c += kFitThreads) {
+        const double v = c < nchans ? bp_all[(size_t)b * nchans + c] : inf;
+        srt[c] = v;
+        if (c < nchans) bp[c] = v;
+    }
+    if (tid == 0) s_nmask = 0;
+    bitonic_sort(srt, npad);
+    const double med = (nchans & 1) ? srt[nchans / 2] : __dmul_rn(0.5, __dadd_rn(srt[nchans / 2 - 1], srt[nchans / 2]));
+    __syncthreads();
+    for (int c = tid; c < npad; c += kFitThreads) srt[c] = c < nchans ? fabs(__dsub_rn(bp[c], med)) : inf;
+    bitonic_sort(srt, npad);
+    const double mad = (nchans & 1) ? srt[nchans / 2] : __dmul_rn(0.5, __dadd_rn(srt[nchans / 2 - 1], srt[nchans / 2]));
+    const double lim = __dmul_rn(__dmul_rn(k_mask, 1.4826), mad);
+    __syncthreads();
+    // H2: mask + interpolate
+    int nm = 0;
+    for (int c = tid; c < nchans; c += kFitThreads) {
+        double v = bp[c];
+        if (__dsub_rn(v, med) > lim) {
+            ++nm;
+            int l = c - 1, r = c + 1;
+            while (l >= 0 && __dsub_rn(bp[l], med) > lim) --l;
+            while (r < nchans && __dsub_rn(bp[r], med) > lim) ++r;
+            if (l >= 0 && r < nchans) v = __dmul_rn(0.5, __dadd_rn(bp[l], bp[r]));
+            else if (l >= 0) v = bp[l];
+            else if (r < nchans) v = bp[r];
+        }
+        bpi[c] = v;
+    }
+    if (nm) atomicAdd(&s_nmask, nm);
+    __syncthreads();
+    // H3: normal equations in u = 2c/(n-1) - 1: sums of u^k (k <= 2p) and of u^k y (k <= p)
+    {
+        double pu[2 * kFitMaxOrder + 1], py[kFitMaxOrder + 1];
+        for (int k = 0; k <= 2 * order; ++k) pu[k] = 0.0;
+        for (int k = 0; k <= order; ++k) py[k] = 0.0;
+        for (int c = tid; c < nchans; c += kFitThreads) {
+            const double u = nchans > 1 ? __dsub_rn(__ddiv_rn(__dmul_rn(2.0, (double)c), (double)(nchans - 1)), 1.0) : 0.0;
+            double pw = 1.0;
+            for (int k = 0; k <= 2 * order; ++k) {
+                pu[k] += pw;
+                if (k <= order) py[k] += pw * bpi[c];
+                pw *= u;
+            }
+        }
+        for (int k = 0; k <= 2 * order; ++k) { const double s = fit_block_sum(pu[k], red); if (tid == 0) sums[k] = s; }
+        for (int k = 0; k <= order; ++k) { const double s = fit_block_sum(py[k], red); if (tid == 0) sums[2 * kFitMaxOrder + 1 + k] = s; }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double A[kFitMaxOrder + 1][kFitMaxOrder + 2];
+        const int p = order;
+        for (int i = 0; i <= p; ++i) {
+            for (int j = 0; j <= p; ++j) A[i][j] = sums[i + j];
+            A[i][p + 1] = sums[2 * kFitMaxOrder + 1 + i];
+        }
+        for (int i = 0; i <= p; ++i) {
+            int piv = i;
+            for (int r = i + 1; r <= p; ++r)
+                if (fabs(A[r][i]) > fabs(A[piv][i])) piv = r;
+            if (piv != i)
+                for (int j = 0; j <= p + 1; ++j) { const double t = A[i][j]; A[i][j] = A[piv][j]; A[piv][j] = t; }
+            for (int r = i + 1; r <= p; ++r) {
+                const double f = A[r][i] / A[i][i];
+                for (int j = i; j <= p + 1; ++j) A[r][j] = __dsub_rn(A[r][j], __dmul_rn(f, A[i][j]));
+            }
+        }
+        for (int i = p; i >= 0; --i) {
+            double s = A[i][p + 1];
+            for (int j = i + 1; j <= p; ++j) s = __dsub_rn(s, __dmul_rn(A[i][j], coef[j]));
+            coef[i] = s / A[i][i];
+        }
+    }
+    __syncthreads();
+    // fit (Horner) and H4
+    double se = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int c = tid; c < nchans; c += kFitThreads) {
+        const double u = nchans > 1 ? __dsub_rn(__ddiv_rn(__dmul_rn(2.0, (double)c), (double)(nchans - 1)), 1.0) : 0.0;
+        double v = coef[order];
+        for (int k = order - 1; k >= 0; --k) v = __dadd_rn(__dmul_rn(v, u), coef[k]);
+        srt[c] = v;                                             // the fit, kept for the second loop (npad >= nchans)
+        const double e = __dsub_rn(v, bpi[c]);
+        se += e * e; s1 += bpi[c]; s2 += bpi[c] * bpi[c];
+    }
+    se = fit_block_sum(se, red);
+    s1 = fit_block_sum(s1, red);
+    s2 = fit_block_sum(s2, red);
+    const double rmse = __dsqrt_rn(__ddiv_rn(se, (double)nchans));
+    const double mean_bp = __ddiv_rn(s1, (double)nchans);
+    double var_bp = __dsub_rn(__ddiv_rn(s2, (double)nchans), __dmul_rn(mean_bp, mean_bp));
+    if (var_bp < 0.0) var_bp = 0.0;
+    const double std_bp = __dsqrt_rn(var_bp);
+    for (int c = tid; c < nchans; c += kFitThreads) {
+        double *st = chan_stats + ((size_t)b * nchans + c) * 4;
+        const double f = srt[c];
+        st[0] = f; st[1] = __dadd_rn(f, __dmul_rn(k_chan, rmse)); st[2] = bpi[c]; st[3] = (double)(float)f;
+        if (out_fit) { out_fit[((size_t)b * nchans + c) * 2] = f; out_fit[((size_t)b * nchans + c) * 2 + 1] = bpi[c]; }
+    }
+    if (tid == 0) {
+        spec_stats[4 * b + 0] = __dadd_rn(mean_bp, __dmul_rn(k_spec, std_bp));
+        spec_stats[4 * b + 1] = rmse; spec_stats[4 * b + 2] = mean_bp; spec_stats[4 * b + 3] = std_bp;
+        if (out_stats) { out_stats[4 * b] = rmse; out_stats[4 * b + 1] = mean_bp; out_stats[4 * b + 2] = std_bp; out_stats[4 * b + 3] = (double)s_nmask; }
+    }
+}
+
+// H6 + H7.  Thread = one time sample x kChPer channels (coalesced along t).
+constexpr int kBpChPer = 16;
+__global__ void __launch_bounds__(kThreads)
+bp_spec_apply_kernel(float *__restrict__ in, int beam0, int nchans, long long nsamps, const double *__restrict__ spec_sum,
+                     const double *__restrict__ spec_stats, const double *__restrict__ chan_stats, int subtract,
+                     uint8_t *__restrict__ spec_mask)
+{
+    const int b = beam0 + blockIdx.z;
+    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (t >= nsamps) return;
+    const bool flag = __ddiv_rn(spec_sum[(size_t)b * nsamps + t], (double)nchans) > spec_stats[4 * b];
+    if (blockIdx.y == 0 && spec_mask) spec_mask[(size_t)b * nsamps + t] = flag ? 1 : 0;
+    if (!flag && !subtract) return;
+    const int c0 = blockIdx.y * kBpChPer, c1 = min(nchans, c0 + kBpChPer);
+    float *col = in + ((size_t)b * nchans + c0) * (size_t)nsamps + t;
+    const double *st = chan_stats + ((size_t)b * nchans + c0) * 4;
+    for (int c = c0; c < c1; ++c, col += nsamps, st += 4) {
+        const float f = (float)st[3];
+        float v = flag ? f : *col;
+        if (subtract) v = v - f;
+        *col = v;
+    }
+}
+
 template <typename T>
 int launch_clip_t(mdsm_plan *p, T *in, int beam0, int nb, int window, double k_chan, double k_spec,
                   uint8_t *chan_mask, uint8_t *spec_mask, cudaStream_t st)
@@ -358,4 +575,55 @@ int mdsm_launch_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int nb, int
     if (dtype == MDSM_F32)
         return launch_clip_t<float>(p, (float *)d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask, d_spec_mask, st);
     return launch_clip_t<uint8_t>(p, (uint8_t *)d_in, beam0, nb, window, k_chan, k_spec, d_chan_mask, d_spec_mask, st);
+}
+
+int mdsm_launch_bandpass_clip(mdsm_plan *p, float *in, int beam0, int nb, int window, int order, double k_mask, double k_chan,
+                              double k_spec, int subtract, uint8_t *chan_mask, uint8_t *spec_mask, double *d_fit, double *d_stats,
+                              cudaStream_t st)
+{
+    const long long nsamps = p->nsamps, nchunk = nsamps / window;
+    const bool aligned = ((uintptr_t)in % 16 == 0) && (nsamps % 4 == 0);
+    int npad = 1;
+    while (npad < p->nchans) npad <<= 1;
+    const size_t fit_smem = (size_t)(2 * p->nchans + npad) * sizeof(double);
+    MDSM_REQUIRE(fit_smem <= 200 * 1024, "bandpass fit: nchans = %d exceeds the shared-memory sort buffer", p->nchans);
+    dim3 grid1(p->nchans, nb);
+    bp_rowmean_kernel<<<grid1, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, aligned ? 1 : 0, p->d_bandpass);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    double *spec_stats = p->d_spec_part;
+    if (fit_smem > 48 * 1024) MDSM_CUDA_TRY(cudaFuncSetAttribute(bp_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fit_smem));
+    bp_fit_kernel<<<nb, kFitThreads, fit_smem, st>>>(p->d_bandpass, beam0, p->nchans, npad, order, k_mask, k_chan, k_spec, p->d_chan_stats,
+                                                    spec_stats, d_fit, d_stats);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    int mode = 2;
+    if (aligned && window % 4 == 0) {
+        const int g = window / 4;
+        if (g <= 32 && (g & (g - 1)) == 0) mode = 0;
+        else if (g % 32 == 0) mode = 1;
+    }
+    size_t smem = (size_t)nchunk + (mode < 2 ? (size_t)nchunk * sizeof(double) : 0);
+    if (mode < 2 && smem > 200 * 1024) { mode = 2; smem = (size_t)nchunk; }
+    MDSM_REQUIRE(smem <= 200 * 1024, "nsamps/window = %lld chunks per channel exceeds the shared-memory flag buffer", nchunk);
+    auto k0 = clip_channel_kernel<float, 0, 1>;
+    auto k1 = clip_channel_kernel<float, 1, 1>;
+    auto k2 = clip_channel_kernel<float, 2, 1>;
+    auto kern = mode == 0 ? k0 : (mode == 1 ? k1 : k2);
+    if (smem > 48 * 1024) MDSM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid1, kThreads, smem, st>>>(in, beam0, p->nchans, nsamps, window, k_chan, p->d_chan_stats, chan_mask);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    if (aligned) {
+        dim3 grid2((unsigned)((nsamps + 32 * 4 - 1) / (32 * 4)), nb);
+        clip_spec_sum_kernel<float, true><<<grid2, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum);
+    } else {
+        dim3 grid2((unsigned)((nsamps + 31) / 32), nb);
+        clip_spec_sum_kernel<float, false><<<grid2, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum);
+    }
+    MDSM_CUDA_TRY(cudaGetLastError());
+    dim3 grid4((unsigned)((nsamps + kThreads - 1) / kThreads), (unsigned)((p->nchans + kBpChPer - 1) / kBpChPer), nb);
+    MDSM_REQUIRE(grid4.y <= 65535 && nb <= 65535, "bandpass stage: grid too large");
+    bp_spec_apply_kernel<<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats, p->d_chan_stats, subtract,
+                                                    spec_mask);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    p->launches += 5;
+    return MDSM_OK;
 }

@@ -73,6 +73,7 @@ struct mdsm_plan {
 
     // clip scratch
     double *d_chan_stats = nullptr;   // [nbeams][nchans][4] = mean, sig, thr(unused), repl
+    double *d_bandpass = nullptr;     // [nbeams][nchans] averaged bandpass (mdsm_bandpass_clip)
     double *d_spec_sum = nullptr;     // [nbeams][nsamps]    spectrum sums (fp64; exact for u8)
     double *d_spec_part = nullptr;    // [nbeams][spec_parts][2] partial M1, M2 (f32 path)
     unsigned long long *d_spec_part_u = nullptr;  // same, integer path
@@ -104,6 +105,9 @@ struct mdsm_plan {
 // stage launchers (each returns an MDSM_* status)
 int mdsm_launch_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int nb, int window, double k_chan,
                      double k_spec, uint8_t *d_chan_mask, uint8_t *d_spec_mask, cudaStream_t st);
+int mdsm_launch_bandpass_clip(mdsm_plan *p, float *in, int beam0, int nb, int window, int order, double k_mask, double k_chan,
+                              double k_spec, int subtract, uint8_t *chan_mask, uint8_t *spec_mask, double *d_fit, double *d_stats,
+                              cudaStream_t st);
 int mdsm_launch_dedisperse_direct(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
                                   cudaStream_t st);
 int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,

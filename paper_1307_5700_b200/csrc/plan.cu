@@ -101,6 +101,7 @@ extern "C" mdsm_plan *mdsm_plan_create(int nbeams, int nchans, double f_top, dou
     p->spec_parts = 256;
     bool ok = alloc_dev((void **)&p->d_delay, p->h_delay.size() * sizeof(int32_t)) &&
               alloc_dev((void **)&p->d_chan_stats, (size_t)nbeams * nchans * 4 * sizeof(double)) &&
+              alloc_dev((void **)&p->d_bandpass, (size_t)nbeams * nchans * sizeof(double)) &&
               alloc_dev((void **)&p->d_spec_sum, (size_t)nbeams * nsamps * sizeof(double)) &&
               alloc_dev((void **)&p->d_spec_part, (size_t)nbeams * p->spec_parts * 2 * sizeof(double)) &&
               alloc_dev((void **)&p->d_spec_part_u, (size_t)nbeams * p->spec_parts * 2 * sizeof(unsigned long long)) &&
@@ -125,6 +126,7 @@ extern "C" void mdsm_plan_destroy(mdsm_plan *p)
     if (!p) return;
     cudaFree(p->d_delay);
     cudaFree(p->d_chan_stats);
+    cudaFree(p->d_bandpass);
     cudaFree(p->d_spec_sum);
     cudaFree(p->d_spec_part);
     cudaFree(p->d_spec_part_u);
@@ -214,6 +216,19 @@ extern "C" int mdsm_rfi_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int
     MDSM_REQUIRE(k_chan == k_chan && k_spec == k_spec, "thresholds must not be NaN");
     return mdsm_launch_clip(p, d_in, dtype, beam0, nb, window, k_chan, k_spec, d_chan_mask, d_spec_mask,
                             (cudaStream_t)cuda_stream);
+}
+
+extern "C" int mdsm_bandpass_clip(mdsm_plan *p, float *d_in, int beam0, int nb, int window, int order, double k_mask,
+                                  double k_chan, double k_spec, int subtract, uint8_t *d_chan_mask, uint8_t *d_spec_mask,
+                                  double *d_fit, double *d_stats, void *cuda_stream)
+{
+    int rc = check_common(p, d_in, MDSM_F32, beam0, nb);
+    if (rc) return rc;
+    MDSM_REQUIRE(window >= 1 && p->nsamps % window == 0, "window must be >= 1 and divide nsamps");
+    MDSM_REQUIRE(order >= 0 && order <= 12 && order < p->nchans, "order must be in [0, 12] and below nchans");
+    MDSM_REQUIRE(k_mask == k_mask && k_chan == k_chan && k_spec == k_spec, "thresholds must not be NaN");
+    return mdsm_launch_bandpass_clip(p, d_in, beam0, nb, window, order, k_mask, k_chan, k_spec, subtract, d_chan_mask, d_spec_mask,
+                                     d_fit, d_stats, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int mdsm_dedisperse(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,

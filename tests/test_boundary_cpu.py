@@ -45,7 +45,7 @@ def test_no_oracle_or_cpu_fallback_in_product_path():
             if f.endswith((".py", ".cu", ".h", ".cuh")):
                 s = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in s and "from oracle" not in s and "mdsm_oracle" not in s, f
-    s = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "mdsm_oracle.c")).read()
+    s = "".join(open(os.path.join(ROOT, "oracle", f)).read() for f in ("__init__.py", "mdsm_oracle.c", "mdsm_oracle_next.c"))
     assert "import paper_1307_5700_b200" not in s and "from paper_1307_5700_b200" not in s and "mdsm.h" not in s
 
 

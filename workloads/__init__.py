@@ -6,4 +6,4 @@ These stand in for the paper's simulated-pulsar benchmark file and BEST-2 record
 the CPU oracle and to the CUDA library; this module is imported by tests/ and bench.py
 and imports neither of them.
 """
-from .configs import CONFIGS, Config, generate, generate_beam, generate_beam_device  # noqa: F401
+from .configs import CONFIGS, Config, generate, generate_beam, generate_beam_device, power_filterbank  # noqa: F401

@@ -216,3 +216,26 @@ def generate_beam_device(cfg: Config, b: int, torch):
             x[:, ts:ts + dur] += 80.0
         return x.round_().clamp_(0.0, 255.0).to(torch.uint8)
     raise ValueError(cfg.recipe)
+
+
+def power_filterbank(nbeams: int, nchans: int, nsamps: int, seed: int, window: int = 64) -> np.ndarray:
+    """Detected-power filterbank for the paper's bandpass-fit RFI stage: exponentially distributed
+    power (one detected sample of a Gaussian voltage) scaled by a smooth telescope bandpass with a small ripple, a few
+    persistent narrow-band RFI channels (the ones the fit must mask), bursts of narrow-band RFI confined to single
+    chunks of `window` samples and a few broadband spikes.  Inputs only: no pipeline arithmetic."""
+    x = np.empty((nbeams, nchans, nsamps), dtype=np.float32)
+    u = np.linspace(-1.0, 1.0, nchans)
+    for b in range(nbeams):
+        g = np.random.default_rng(seed + b)
+        bp = 10.0 * (1.0 - 0.35 * u * u + 0.1 * u + 0.05 * u ** 3) * (1.0 + 0.01 * np.sin(40.0 * u + g.uniform(0, 6.28)))
+        xb = g.exponential(size=(nchans, nsamps)).astype(np.float32) * bp[:, None].astype(np.float32)
+        for c in g.choice(nchans, size=max(1, nchans // 100), replace=False):
+            xb[c] *= np.float32(g.uniform(3.0, 8.0))                        # persistent RFI channels
+        nchunk = nsamps // window
+        for _ in range(max(2, nchans // 20)):
+            c, j = int(g.integers(nchans)), int(g.integers(nchunk))
+            xb[c, j * window:(j + 1) * window] += np.float32(bp[c] * g.uniform(1.0, 4.0))   # bursts
+        for _ in range(5):
+            xb[:, int(g.integers(nsamps))] += (bp * g.uniform(3.0, 6.0)).astype(np.float32)  # broadband spikes
+        x[b] = xb
+    return x

@@ -180,6 +180,31 @@ int mdsm_power_i16(const int16_t *d_volt, float *d_power, int64_t n, void *cuda_
  * n < 0 or mu <= 0. */
 int mdsm_mulaw_u8(const float *d_x, uint8_t *d_code, int64_t n, double mu, float *d_xmax, void *cuda_stream);
 
+/* Host candidate stage (north_star: "clustering and the analytic DM-SNR candidate
+ * filter stay on the host").  Both calls take HOST pointers, run on the calling thread and need neither a plan nor a GPU.
+ *
+ * mdsm_cluster_events: density clustering of detections in (time [samples], DM [pc cm^-3], SNR), beam by beam
+ *   (one list per beam).  q is a neighbour of p when |dt| <= eps_t, |dDM| <= eps_dm and |dSNR| <= eps_snr
+ *   ("a different value to each dimension (T_t, SNR_t, DM_t)"); a core point has >= min_pts neighbours,
+ *   itself included.  exact = 0: FDBSCAN: only the representative border points of a core point's
+ *   neighbourhood (per dimension and direction the farthest neighbour of this cluster) are expanded; exact = 1: DBSCAN.
+ *   h_labels[i] receives the cluster id of event i (0 .. *h_nclusters - 1, numbered beam by beam in order of discovery)
+ *   or -1 (noise); *h_nqueries (may be NULL) the number of neighbourhood queries made.  DM of an event =
+ *   dm_low + dm_idx * dm_step.
+ * mdsm_classify_clusters: the eight steps of PAPER.md:144-156 per cluster: DM-SNR signature (strongest detection per DM),
+ *   k_smooth-element moving average (odd), the DM with the most detections (DM < 1.0 => broadband RFI), the pulse width
+ *   at that DM, normalisation, the model curve of Eq. 3 with zeta of Eq. 4 (bw_mhz = bandwidth, nu_ghz = centre
+ *   frequency), the RMSE between the two, RMSE > rmse_max => RFI.
+ *   h_results [nclusters][5] = class (0 candidate, 1 RFI: DM < 1, 2 RFI: curve mismatch, -1 empty cluster id),
+ *   dm_idx of the peak, its SNR, width in ms, RMSE.
+ * MDSM_EINVAL for null pointers / non-positive eps / even k_smooth / labels out of range. */
+int mdsm_cluster_events(const mdsm_event *h_events, int64_t n, double dm_low, double dm_step, double eps_t,
+                        double eps_dm, double eps_snr, int min_pts, int exact, int32_t *h_labels,
+                        int64_t *h_nclusters, int64_t *h_nqueries);
+int mdsm_classify_clusters(const mdsm_event *h_events, const int32_t *h_labels, int64_t n, int64_t nclusters,
+                           double dm_low, double dm_step, double tsamp, double bw_mhz, double nu_ghz, int k_smooth,
+                           double rmse_max, double *h_results);
+
 /* The whole chain from HOST buffers (per-beam threads copy their input to the GPU;
  * north_star item 4: beam groups on separate CUDA streams with overlapped host-to-device copies).
  * h_in [nbeams][nchans][nsamps] (pinned memory overlaps best); the clipped data is NOT copied back.

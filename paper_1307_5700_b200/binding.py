@@ -19,6 +19,7 @@ __all__ = [
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
     "mdsm_plan_reserve", "mdsm_plan_kernel_info",
     "mdsm_rfi_clip", "mdsm_bandpass_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
+    "mdsm_cluster_events", "mdsm_classify_clusters",
 ]
 
 MDSM_F32, MDSM_U8 = 0, 1
@@ -83,6 +84,12 @@ def _load():
     L.mdsm_power_i16.argtypes = [c_void_p, c_void_p, c_int64, c_void_p]
     L.mdsm_mulaw_u8.restype = c_int
     L.mdsm_mulaw_u8.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]
+    L.mdsm_cluster_events.restype = c_int
+    L.mdsm_cluster_events.argtypes = [c_void_p, c_int64, c_double, c_double, c_double, c_double, c_double, c_int, c_int, c_void_p,
+                                      POINTER(c_int64), POINTER(c_int64)]
+    L.mdsm_classify_clusters.restype = c_int
+    L.mdsm_classify_clusters.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_double, c_double, c_double, c_double, c_double,
+                                         c_int, c_double, c_void_p]
     L.mdsm_pipeline_host.restype = c_int
     L.mdsm_pipeline_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, c_double, c_void_p,
                                      c_int64, POINTER(c_uint64), c_int]
@@ -241,3 +248,24 @@ def mdsm_measure_add_peak(kind: int) -> float:
     v = c_double(0.0)
     _check(_L.mdsm_measure_add_peak(kind, ctypes.byref(v)))
     return float(v.value)
+
+
+def mdsm_cluster_events(h_events: np.ndarray, dm_low, dm_step, eps_t, eps_dm, eps_snr, min_pts, exact=False):
+    """Host FDBSCAN / DBSCAN of an EVENT_DTYPE array. Returns (labels int32 [n], nclusters, region queries)."""
+    ev = np.ascontiguousarray(h_events, dtype=EVENT_DTYPE)
+    labels = np.empty(ev.shape[0], dtype=np.int32)
+    ncl, nq = c_int64(0), c_int64(0)
+    _check(_L.mdsm_cluster_events(ev.ctypes.data, ev.shape[0], dm_low, dm_step, eps_t, eps_dm, eps_snr, min_pts,
+                                  1 if exact else 0, labels.ctypes.data, ctypes.byref(ncl), ctypes.byref(nq)))
+    return labels, int(ncl.value), int(nq.value)
+
+
+def mdsm_classify_clusters(h_events: np.ndarray, h_labels: np.ndarray, nclusters, dm_low, dm_step, tsamp, bw_mhz, nu_ghz,
+                           k_smooth, rmse_max) -> np.ndarray:
+    """Host DM-SNR classifier. Returns [nclusters][5] = class, dm_idx, snr, width_ms, rmse."""
+    ev = np.ascontiguousarray(h_events, dtype=EVENT_DTYPE)
+    lab = np.ascontiguousarray(h_labels, dtype=np.int32)
+    res = np.zeros((nclusters, 5), dtype=np.float64)
+    _check(_L.mdsm_classify_clusters(ev.ctypes.data, lab.ctypes.data, ev.shape[0], nclusters, dm_low, dm_step, tsamp, bw_mhz,
+                                     nu_ghz, k_smooth, rmse_max, res.ctypes.data))
+    return res

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdsm.so")
-SOURCES = ["plan.cu", "clip.cu", "dedisperse_direct.cu", "dedisperse_rows.cu", "detect.cu", "postprocess.cu", "power.cu", "mulaw.cu", "pipeline.cu", "add_peak.cu"]
+SOURCES = ["plan.cu", "clip.cu", "dedisperse_direct.cu", "dedisperse_rows.cu", "detect.cu", "postprocess.cu", "power.cu", "mulaw.cu", "pipeline.cu", "add_peak.cu", "candidates.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-O2,-ffp-contract=off", "-shared",

@@ -40,7 +40,10 @@ typedef struct mdsm_plan mdsm_plan;                                 /* opaque */
 /* One detection: "(time, DM, intensity) triplets" per beam.  16 bytes. */
 typedef struct { int32_t beam, dm_idx, t; float snr; } mdsm_event;
 
-enum { MDSM_F32 = 0, MDSM_U8 = 1 };
+/* Sample types.  MDSM_F32 and MDSM_U8 are accepted by every stage call; MDSM_U16 (uint16 samples) and MDSM_U4 (4-bit samples,
+ * two per byte along time, low nibble first; nsamps even) are further INPUT types of mdsm_dedisperse only (SURVEY 8(f)
+ * NEXT-4: lower-precision inputs), with uint32 output like MDSM_U8 -- pass MDSM_U8 to mdsm_detect for their series. */
+enum { MDSM_F32 = 0, MDSM_U8 = 1, MDSM_U16 = 2, MDSM_U4 = 3 };
 enum { MDSM_OK = 0, MDSM_EINVAL = -1, MDSM_ENOMEM = -2, MDSM_ECUDA = -3, MDSM_EOVERFLOW = 1 };
 
 /* Survey parameters of one buffer (PAPER.md:96 "observation and survey parameters", :190, :194).
@@ -129,7 +132,8 @@ int mdsm_bandpass_clip(mdsm_plan *plan, float *d_in, int beam0, int nb, int wind
 /* Brute-force incoherent dedispersion:
  *   out[b][d][t] = sum_c in[b][c][t + delay(d,c)],   t in [0, nsamps_out)
  * MDSM_F32: float in, float out (fp32 accumulation; |err| <= 1e-5 * sum_c|in| + 1e-6).
- * MDSM_U8 : uint8 in, uint32 out, exact.
+ * MDSM_U8 : uint8 in, uint32 out, exact.  MDSM_U16: uint16 in, uint32 out, exact (nchans * 65535 must fit 32 bits).
+ * MDSM_U4 : 4-bit samples packed two per byte (row = nsamps/2 bytes), uint32 out, exact.
  * d_in [nbeams][nchans][nsamps], d_out [nbeams][ndms][nsamps] (only t < nsamps_out of the rows of beams
  * [beam0, beam0+nb) is written), both caller-owned device buffers of any alignment.  Asynchronous on cuda_stream;
  * allocates nothing: the scratch of the pre-summed-rows kernel must have been reserved with
@@ -179,6 +183,15 @@ int mdsm_power_i16(const int16_t *d_volt, float *d_power, int64_t n, void *cuda_
  * (the decoder needs it).  Asynchronous on cuda_stream; needs no plan.  MDSM_EINVAL for null / misaligned buffers,
  * n < 0 or mu <= 0. */
 int mdsm_mulaw_u8(const float *d_x, uint8_t *d_code, int64_t n, double mu, float *d_xmax, void *cuda_stream);
+
+/* mu-law quantiser of the 16-bit complex channelised voltages to 2 x 4 bits per sample ("16-bit complex
+ * values are quantized to 4-bits with two complex components packed into one byte"; Eq. 5; Fig. 5b; reading G-ii):
+ *   Xmax = max |component| of the buffer;  code(v) = sign(v) * floor(7 * log(1 + mu |v| / Xmax) / log(1 + mu) + 0.5) in [-7, 7];
+ *   packed[i] = (code(re_i) & 15) | (code(im_i) & 15) << 4   (two's-complement nibbles; Xmax = 0 -> zeros).
+ * d_volt [n][2] int16 (re, im), d_packed [n] bytes, both 16-byte aligned device buffers; d_xmax_thr: nine device int32 that
+ * receive Xmax and the law as integer thresholds (thr[k] = smallest |v| with code >= k + 1, k < 7; the decoder's table).
+ * Asynchronous on cuda_stream; needs no plan.  MDSM_EINVAL for null / misaligned buffers, n < 0 or mu <= 0. */
+int mdsm_mulaw_c4(const int16_t *d_volt, uint8_t *d_packed, int64_t n, double mu, int32_t *d_xmax_thr, void *cuda_stream);
 
 /* Host candidate stage (north_star: "clustering and the analytic DM-SNR candidate
  * filter stay on the host").  Both calls take HOST pointers, run on the calling thread and need neither a plan nor a GPU.

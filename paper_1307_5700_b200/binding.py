@@ -13,16 +13,16 @@ from ctypes import (POINTER, c_char_p, c_double, c_int, c_int32, c_int64, c_uint
 import numpy as np
 
 __all__ = [
-    "MDSM_F32", "MDSM_U8", "MDSM_OK", "MDSM_EINVAL", "MDSM_ENOMEM", "MDSM_ECUDA", "MDSM_EOVERFLOW",
+    "MDSM_F32", "MDSM_U8", "MDSM_U16", "MDSM_U4", "MDSM_OK", "MDSM_EINVAL", "MDSM_ENOMEM", "MDSM_ECUDA", "MDSM_EOVERFLOW",
     "EVENT_DTYPE", "MdsmError", "lib_path",
     "mdsm_plan_create", "mdsm_plan_destroy", "mdsm_plan_max_delay", "mdsm_plan_nsamps_out",
     "mdsm_plan_get_delays", "mdsm_last_error", "mdsm_plan_set_option", "mdsm_plan_launch_count",
     "mdsm_plan_reserve", "mdsm_plan_kernel_info",
     "mdsm_rfi_clip", "mdsm_bandpass_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
-    "mdsm_cluster_events", "mdsm_classify_clusters",
+    "mdsm_cluster_events", "mdsm_classify_clusters", "mdsm_mulaw_c4",
 ]
 
-MDSM_F32, MDSM_U8 = 0, 1
+MDSM_F32, MDSM_U8, MDSM_U16, MDSM_U4 = 0, 1, 2, 3
 MDSM_OK, MDSM_EINVAL, MDSM_ENOMEM, MDSM_ECUDA, MDSM_EOVERFLOW = 0, -1, -2, -3, 1
 EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
 
@@ -84,6 +84,8 @@ def _load():
     L.mdsm_power_i16.argtypes = [c_void_p, c_void_p, c_int64, c_void_p]
     L.mdsm_mulaw_u8.restype = c_int
     L.mdsm_mulaw_u8.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]
+    L.mdsm_mulaw_c4.restype = c_int
+    L.mdsm_mulaw_c4.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]
     L.mdsm_cluster_events.restype = c_int
     L.mdsm_cluster_events.argtypes = [c_void_p, c_int64, c_double, c_double, c_double, c_double, c_double, c_int, c_int, c_void_p,
                                       POINTER(c_int64), POINTER(c_int64)]
@@ -131,6 +133,8 @@ def _dtype_of(x, dtype):
         return MDSM_F32
     if name.endswith("uint8") or name.endswith("uint32") or name.endswith("int32"):
         return MDSM_U8
+    if name.endswith("uint16") or name.endswith("int16"):
+        return MDSM_U16
     raise TypeError(f"cannot infer mdsm dtype from {name!r}")
 
 
@@ -248,6 +252,10 @@ def mdsm_measure_add_peak(kind: int) -> float:
     v = c_double(0.0)
     _check(_L.mdsm_measure_add_peak(kind, ctypes.byref(v)))
     return float(v.value)
+
+
+def mdsm_mulaw_c4(d_volt, d_packed, n, mu, d_xmax_thr, stream=None) -> None:
+    _check(_L.mdsm_mulaw_c4(_ptr(d_volt), _ptr(d_packed), n, mu, _ptr(d_xmax_thr), _stream(stream)))
 
 
 def mdsm_cluster_events(h_events: np.ndarray, dm_low, dm_step, eps_t, eps_dm, eps_snr, min_pts, exact=False):

@@ -10,7 +10,8 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kPer = 4;
 
-template <typename TIn, typename TOut>
+// U4: TIn = uint8_t holds two 4-bit samples per byte along time (low nibble first); a row is nsamps / 2 bytes
+template <typename TIn, typename TOut, bool U4 = false>
 __global__ void __launch_bounds__(kThreads)
 dedisperse_direct_kernel(const TIn *__restrict__ in, TOut *__restrict__ out, const int32_t *__restrict__ delay,
                          int beam0, int nchans, int ndms, long long nsamps, long long nsamps_out)
@@ -21,7 +22,8 @@ dedisperse_direct_kernel(const TIn *__restrict__ in, TOut *__restrict__ out, con
     for (int c = threadIdx.x; c < nchans; c += kThreads) sdelay[c] = delay[(size_t)d * nchans + c];
     __syncthreads();
     const long long t0 = (long long)blockIdx.x * (kThreads * kPer) + threadIdx.x;
-    const TIn *base = in + (size_t)b * nchans * (size_t)nsamps;
+    const size_t row_elems = U4 ? (size_t)nsamps / 2 : (size_t)nsamps;
+    const TIn *base = in + (size_t)b * nchans * row_elems;
     TOut acc[kPer];
     bool ok[kPer];
 #pragma unroll
@@ -30,10 +32,21 @@ dedisperse_direct_kernel(const TIn *__restrict__ in, TOut *__restrict__ out, con
         ok[k] = t0 + k * kThreads < nsamps_out;
     }
     for (int c = 0; c < nchans; ++c) {
-        const TIn *row = base + (size_t)c * nsamps + sdelay[c] + t0;
+        if constexpr (U4) {
+            const TIn *row = base + (size_t)c * row_elems;
+            const long long s0 = sdelay[c] + t0;
 #pragma unroll
-        for (int k = 0; k < kPer; ++k)
-            if (ok[k]) acc[k] += (TOut)row[k * kThreads];
+            for (int k = 0; k < kPer; ++k)
+                if (ok[k]) {
+                    const long long sidx = s0 + k * kThreads;
+                    acc[k] += (TOut)((row[sidx >> 1] >> (4 * (int)(sidx & 1))) & 15);
+                }
+        } else {
+            const TIn *row = base + (size_t)c * nsamps + sdelay[c] + t0;
+#pragma unroll
+            for (int k = 0; k < kPer; ++k)
+                if (ok[k]) acc[k] += (TOut)row[k * kThreads];
+        }
     }
     TOut *orow = out + ((size_t)b * ndms + d) * (size_t)nsamps + t0;
 #pragma unroll
@@ -53,8 +66,14 @@ int mdsm_launch_dedisperse_direct(mdsm_plan *p, const void *d_in, int dtype, int
     if (dtype == MDSM_F32)
         dedisperse_direct_kernel<float, float><<<grid, kThreads, smem, st>>>(
             (const float *)d_in, (float *)d_out, p->d_delay, beam0, p->nchans, p->ndms, p->nsamps, p->nsamps_out);
-    else
+    else if (dtype == MDSM_U8)
         dedisperse_direct_kernel<uint8_t, uint32_t><<<grid, kThreads, smem, st>>>(
+            (const uint8_t *)d_in, (uint32_t *)d_out, p->d_delay, beam0, p->nchans, p->ndms, p->nsamps, p->nsamps_out);
+    else if (dtype == MDSM_U16)
+        dedisperse_direct_kernel<uint16_t, uint32_t><<<grid, kThreads, smem, st>>>(
+            (const uint16_t *)d_in, (uint32_t *)d_out, p->d_delay, beam0, p->nchans, p->ndms, p->nsamps, p->nsamps_out);
+    else
+        dedisperse_direct_kernel<uint8_t, uint32_t, true><<<grid, kThreads, smem, st>>>(
             (const uint8_t *)d_in, (uint32_t *)d_out, p->d_delay, beam0, p->nchans, p->ndms, p->nsamps, p->nsamps_out);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 1;

@@ -101,35 +101,36 @@ struct PreArgs {
 // fp32: one CTA = one channel group x one chunk of kPreChunkF32 samples x one beam.  The G raw rows of the chunk (plus
 // the largest delta) go to shared memory once and serve every pattern of the group; thread `tid` owns the samples
 // tid + 256 k, so that the shifted reads are conflict-free at any delta and the y stores are coalesced.
-template <int G>
-__global__ void __launch_bounds__(kPreThreads) group_presum_f32_kernel(const PreArgs a)
+// TIn/TOut = float/float (MDSM_F32) or uint16/uint32 (MDSM_U16: the same 32-bit rows with integer sums).
+template <int G, typename TIn, typename TOut>
+__global__ void __launch_bounds__(kPreThreads) group_presum_w32_kernel(const PreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float *sm = reinterpret_cast<float *>(smem_raw);
+    TOut *sm = reinterpret_cast<TOut *>(smem_raw);
     const int g = blockIdx.y, b = a.beam0 + blockIdx.z;
     const int c0 = g * a.G;
     const long long t0 = (long long)blockIdx.x * kPreChunkF32;
     const int pitch = kPreChunkF32 + a.dmax;
-    const float *in = reinterpret_cast<const float *>(a.in) + (size_t)b * a.nchans * (size_t)a.nsamps;
+    const TIn *in = reinterpret_cast<const TIn *>(a.in) + (size_t)b * a.nchans * (size_t)a.nsamps;
 #pragma unroll
     for (int i = 0; i < G; ++i) {
         const bool have = c0 + i < a.nchans;
-        const float *row = in + (size_t)(have ? c0 + i : 0) * a.nsamps;
-        for (int s = threadIdx.x; s < pitch; s += kPreThreads) sm[i * pitch + s] = (have && t0 + s < a.nsamps) ? row[t0 + s] : 0.0f;
+        const TIn *row = in + (size_t)(have ? c0 + i : 0) * a.nsamps;
+        for (int s = threadIdx.x; s < pitch; s += kPreThreads) sm[i * pitch + s] = (have && t0 + s < a.nsamps) ? (TOut)row[t0 + s] : (TOut)0;
     }
     __syncthreads();
     const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
-    float *ybeam = reinterpret_cast<float *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
+    TOut *ybeam = reinterpret_cast<TOut *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
     for (int r = row0; r < row1; ++r) {
         int dl[G];
 #pragma unroll
         for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
-        float *yrow = ybeam + (size_t)r * a.ystride + t0;
-        float v[kPreChunkF32 / kPreThreads];
+        TOut *yrow = ybeam + (size_t)r * a.ystride + t0;
+        TOut v[kPreChunkF32 / kPreThreads];
 #pragma unroll
         for (int k = 0; k < kPreChunkF32 / kPreThreads; ++k) {
             const int s = threadIdx.x + k * kPreThreads;
-            float acc = sm[s];                                   // delta_0 = 0
+            TOut acc = sm[s];                                    // delta_0 = 0
 #pragma unroll
             for (int i = 1; i < G; ++i) acc += sm[i * pitch + s + dl[i]];
             v[k] = acc;
@@ -197,6 +198,51 @@ __global__ void __launch_bounds__(kPreThreads) group_presum_u8_kernel(const PreA
     }
 }
 
+
+// 4-bit samples (two per byte along time, low nibble first) -> uint16 group sums.  Thread `tid` owns the samples
+// 4 (tid + 256 k) .. +3: the four nibbles of row i at delta_i are 16 bits starting at nibble s + delta_i, cut out of two
+// aligned words with one funnel shift and spread to two u16x2 words.
+template <int G>
+__global__ void __launch_bounds__(kPreThreads) group_presum_u4_kernel(const PreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int g = blockIdx.y, b = a.beam0 + blockIdx.z;
+    const int c0 = g * a.G;
+    const long long t0 = (long long)blockIdx.x * kPreChunkU8;                   // samples; t0 / 2 bytes into the row
+    const int pitch = (((kPreChunkU8 + a.dmax) / 2 + 3) & ~3) + 8;               // bytes, whole words, room for the two-word fetch
+    const long long row_bytes = a.nsamps / 2;
+    const uint8_t *in = reinterpret_cast<const uint8_t *>(a.in) + (size_t)b * a.nchans * (size_t)row_bytes;
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const bool have = c0 + i < a.nchans;
+        const uint8_t *row = in + (size_t)(have ? c0 + i : 0) * row_bytes;
+        for (int s = threadIdx.x; s < pitch; s += kPreThreads) smem_raw[i * pitch + s] = (have && t0 / 2 + s < row_bytes) ? row[t0 / 2 + s] : (uint8_t)0;
+    }
+    __syncthreads();
+    const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    uint16_t *ybeam = reinterpret_cast<uint16_t *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
+    for (int r = row0; r < row1; ++r) {
+        int dl[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        uint16_t *yrow = ybeam + (size_t)r * a.ystride + t0;
+#pragma unroll
+        for (int k = 0; k < kPreChunkU8 / (4 * kPreThreads); ++k) {
+            const int s = 4 * (threadIdx.x + k * kPreThreads);
+            uint32_t lo = 0, hi = 0;
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int nib = s + dl[i];                                      // first nibble of the four
+                const uint32_t *w = reinterpret_cast<const uint32_t *>(smem_raw + i * pitch + ((nib >> 1) & ~3));
+                const uint32_t v = __funnelshift_r(w[0], w[1], 4 * (nib & 7));
+                lo += (v & 0xfu) | ((v & 0xf0u) << 12);
+                hi += ((v >> 8) & 0xfu) | ((v & 0xf000u) << 4);
+            }
+            if (t0 + s < a.ystride) *reinterpret_cast<uint2 *>(yrow + s) = make_uint2(lo, hi);
+        }
+    }
+}
+
 // ------------------------------------------------------------------ step 2: the sum of shifted rows
 struct RowsArgs {
     const void *y;                    // [nslots][nyrows][ystride] pre-summed rows
@@ -210,9 +256,12 @@ struct RowsArgs {
     long long ntiles, nsamps, nsamps_out, ystride;
 };
 
-template <int D_, int T_, int NW_, bool F32_> struct RowsTraits {
+// F32_: 32-bit rows, one sample per word (INT_ = false: float adds, MDSM_F32; INT_ = true: integer adds, MDSM_U16);
+// !F32_: 16-bit rows packed two per word (MDSM_U8, MDSM_U4).
+template <int D_, int T_, int NW_, bool F32_, bool INT_ = false> struct RowsTraits {
     static constexpr int D = D_, T = T_, NW = NW_;
     static constexpr bool kF32 = F32_;
+    using Acc = typename std::conditional<INT_, uint32_t, float>::type;
     static constexpr int kSpan = F32_ ? 32 * T_ : 64 * T_;          // samples a warp's accumulators cover per DM
     using Y = typename std::conditional<F32_, float, uint16_t>::type;
 };
@@ -294,11 +343,12 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
         const long long tile_t0 = (long long)tt * a.stride;
         const int b = a.beam0 + bb;
         if constexpr (Tr::kF32) {
-            float acc[D][T];
+            using Acc = typename Tr::Acc;
+            Acc acc[D][T];
 #pragma unroll
             for (int j = 0; j < D; ++j)
 #pragma unroll
-                for (int i = 0; i < T; ++i) acc[j][i] = 0.0f;
+                for (int i = 0; i < T; ++i) acc[j][i] = (Acc)0;
 #pragma unroll 1
             for (int slab = 0; slab < a.nslab; ++slab) {
                 const int nq = min(Q, a.ngroups - slab * Q);
@@ -312,8 +362,8 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
                     for (int j = 0; j < D; ++j) e[j] = ents[j * Q + q];
 #pragma unroll
                     for (int j = 0; j < D; ++j) {
-                        const float *w = reinterpret_cast<const float *>(sbase + e[j]) + lane;
-                        float v[T];
+                        const Acc *w = reinterpret_cast<const Acc *>(sbase + e[j]) + lane;
+                        Acc v[T];
 #pragma unroll
                         for (int i = 0; i < T; ++i) v[i] = w[32 * i];
 #pragma unroll
@@ -329,7 +379,7 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
                 const int dl = warp * D + j, d = blk * DB + dl;
                 if (d >= a.ndms) continue;
                 const int sg = a.sigma[dl];
-                float *orow = reinterpret_cast<float *>(a.out) + ((size_t)b * a.ndms + d) * (size_t)a.nsamps;
+                Acc *orow = reinterpret_cast<Acc *>(a.out) + ((size_t)b * a.ndms + d) * (size_t)a.nsamps;
 #pragma unroll
                 for (int i = 0; i < T; ++i) {
                     const long long t = tile_t0 - sg + lane + 32 * i;
@@ -681,7 +731,8 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
 struct RowsGeom { int D, T, NW; };
 constexpr RowsGeom kGeomRowsF32 = {4, 16, 16};      // 64 DMs x 512 samples per tile
 constexpr RowsGeom kGeomRowsU16 = {4, 8, 16};       // 64 DMs x 512 samples (504 owned) per tile
-constexpr int kPartChans = 256;                     // 256 * 255 < 2^16: the most channels a 16-bit lane can take
+constexpr int kPartChansU8 = 256;                   // 256 * 255 < 2^16: the most uint8 channels a 16-bit lane can take
+constexpr int kPartChansU4 = 4096;                  // 4096 * 15 < 2^16: the same for 4-bit samples
 constexpr size_t kSmemBudget = 227 * 1024;
 
 static inline long long floor_to(long long v, int a) { return v >= 0 ? (v / a) * a : -(((-v) + a - 1) / a) * a; }
@@ -751,7 +802,7 @@ struct RowsHost {
 };
 
 // Builds the per-block staging lists and entry tables for one dtype, group size and geometry.
-static bool build_rows_tables(const mdsm_plan *p, bool f32, const GroupRows &gr, const RowsGeom &g, RowsTables &rt, RowsHost &h)
+static bool build_rows_tables(const mdsm_plan *p, bool f32, int part_chans, const GroupRows &gr, const RowsGeom &g, RowsTables &rt, RowsHost &h)
 {
     const int al = f32 ? 4 : 8, esize = f32 ? 4 : 2;
     const int DB = g.D * g.NW;
@@ -786,7 +837,7 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, const GroupRows &gr,
         }
     const int pitch = (int)ceil_to(need_max, al);
     // groups per slab: as many as keep a slab within 32 rows (one per producer lane) and three stages in shared memory
-    const int part_groups_max = f32 ? ng : std::max(1, kPartChans / G);
+    const int part_groups_max = f32 ? ng : std::max(1, part_chans / G);
     int Q = 0, CS = 0;
     for (int q : {4, 3, 2, 1}) {
         if (!f32 && part_groups_max % q) continue;
@@ -1000,9 +1051,10 @@ static void free_rows_tables(RowsTables *rt)
 // main kernel, plus the y rows, each written to and read back from HBM (about 14 word-times per row and sample).
 static double group_cost(const mdsm_plan *p, const GroupRows &gr) { return (double)p->ndms * gr.ngroups + 14.0 * gr.nyrows; }
 
-static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &cands)
+static int build_dtype(mdsm_plan *p, int kind /* 0: 32-bit rows, 1: uint8 -> 16-bit rows, 2: 4-bit -> 16-bit rows */, const std::vector<GroupRows> &cands)
 {
-    RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
+    const bool f32 = kind == 0;
+    RowsTables &rt = kind == 0 ? p->rows_f32 : (kind == 1 ? p->rows_u8 : p->rows_u4);
     free_rows_tables(&rt);
     if (f32) free_tmem_tables(&p->tmem_f32);
     const RowsGeom geom = f32 ? kGeomRowsF32 : kGeomRowsU16;
@@ -1012,7 +1064,7 @@ static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &can
     std::sort(order.begin(), order.end(), [&](const GroupRows *x, const GroupRows *y) { return group_cost(p, *x) < group_cost(p, *y); });
     for (const GroupRows *gr : order) {
         RowsHost h;
-        if (!build_rows_tables(p, f32, *gr, geom, rt, h)) continue;
+        if (!build_rows_tables(p, f32, kind == 2 ? kPartChansU4 : kPartChansU8, *gr, geom, rt, h)) continue;
         if (!upload((int4 **)&rt.d_rowdesc, h.rowdesc) || !upload(&rt.d_ent, h.ent) || !upload(&rt.d_sigma, h.sigma) ||
             !upload(&rt.d_group_row0, gr->group_row0) || !upload(&rt.d_ydelta, gr->ydelta)) {
             mdsm_set_error("dedispersion table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -1040,10 +1092,24 @@ static int build_dtype(mdsm_plan *p, bool f32, const std::vector<GroupRows> &can
     return MDSM_OK;                                                    // no table: the direct kernel runs
 }
 
-template <int G> static void launch_presum(bool f32, const PreArgs &a, dim3 grid, size_t smem, cudaStream_t st)
+template <int G> static cudaError_t launch_presum(int dtype, const PreArgs &a, dim3 grid, size_t smem, cudaStream_t st)
 {
-    if (f32) group_presum_f32_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
-    else group_presum_u8_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
+    cudaError_t e = cudaSuccess;
+    // only very wide groups need more than the default dynamic shared memory; set per launch (per-device state)
+    if (dtype == MDSM_F32) {
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(group_presum_w32_kernel<G, float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) group_presum_w32_kernel<G, float, float><<<grid, kPreThreads, smem, st>>>(a);
+    } else if (dtype == MDSM_U16) {
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(group_presum_w32_kernel<G, uint16_t, uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) group_presum_w32_kernel<G, uint16_t, uint32_t><<<grid, kPreThreads, smem, st>>>(a);
+    } else if (dtype == MDSM_U8) {
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(group_presum_u8_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) group_presum_u8_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
+    } else {
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(group_presum_u4_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) group_presum_u4_kernel<G><<<grid, kPreThreads, smem, st>>>(a);
+    }
+    return e;
 }
 
 template <typename Tr> static int launch_rows(const RowsArgs &a, size_t smem, int grid, cudaStream_t st)
@@ -1066,8 +1132,9 @@ int mdsm_rows_build_tables(mdsm_plan *p)
         GroupRows gr;
         if (enumerate_group_rows(p, G, gr)) cands.push_back(std::move(gr));
     }
-    int rc = build_dtype(p, true, cands);
-    if (rc == MDSM_OK) rc = build_dtype(p, false, cands);
+    int rc = build_dtype(p, 0, cands);
+    if (rc == MDSM_OK) rc = build_dtype(p, 1, cands);
+    if (rc == MDSM_OK) rc = build_dtype(p, 2, cands);
     return rc;
 }
 
@@ -1076,24 +1143,26 @@ void mdsm_rows_free_tables(mdsm_plan *p)
     free_tmem_tables(&p->tmem_f32);
     free_rows_tables(&p->rows_f32);
     free_rows_tables(&p->rows_u8);
+    free_rows_tables(&p->rows_u4);
 }
 
 size_t mdsm_rows_scratch_bytes_per_beam(const mdsm_plan *p, int dtype)
 {
-    const RowsTables &rt = dtype == MDSM_F32 ? p->rows_f32 : p->rows_u8;
-    return rt.ok ? (size_t)rt.nyrows * (size_t)rt.ystride * (dtype == MDSM_F32 ? 4 : 2) : 0;
+    const RowsTables &rt = mdsm_rows_of(p, dtype);
+    return rt.ok ? (size_t)rt.nyrows * (size_t)rt.ystride * ((dtype == MDSM_F32 || dtype == MDSM_U16) ? 4 : 2) : 0;
 }
 
 int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out, cudaStream_t st)
 {
-    const bool f32 = dtype == MDSM_F32;
-    const RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
-    void *scratch = f32 ? p->d_scratch_f32 : p->d_scratch_u8;
-    const int nslots = f32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
+    const bool f32 = dtype == MDSM_F32, w32 = dtype == MDSM_F32 || dtype == MDSM_U16;
+    const RowsTables &rt = mdsm_rows_of(p, dtype);
+    void *scratch = p->d_scratch[dtype];
+    const int nslots = p->scratch_slots[dtype];
     MDSM_REQUIRE(rt.ok && scratch && nslots >= 1, "dedispersion scratch not reserved (call mdsm_plan_reserve)");
     const int ntile_t = (int)((p->nsamps_out + rt.sigma_max + rt.stride - 1) / rt.stride);
-    const int chunk = f32 ? kPreChunkF32 : kPreChunkU8;
-    const size_t pre_smem = f32 ? (size_t)rt.G * (chunk + rt.dmax) * sizeof(float) : (size_t)rt.G * (chunk + ((rt.dmax + 3) & ~3) + 4);
+    const int chunk = w32 ? kPreChunkF32 : kPreChunkU8;
+    const size_t pre_smem = w32 ? (size_t)rt.G * (chunk + rt.dmax) * 4
+                                : (dtype == MDSM_U8 ? (size_t)rt.G * (chunk + ((rt.dmax + 3) & ~3) + 4) : (size_t)rt.G * ((((chunk + rt.dmax) / 2 + 3) & ~3) + 8));
     MDSM_REQUIRE(pre_smem <= 200 * 1024, "pre-pass: group delay range too large");
     // beams go through the scratch `nslots` at a time (slot = beam % nslots), in stream order
     for (int bs = beam0; bs < beam0 + nb; bs += nslots) {
@@ -1104,26 +1173,18 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
         pa.nsamps = p->nsamps; pa.ystride = rt.ystride;
         dim3 grid((unsigned)((rt.ystride + chunk - 1) / chunk), rt.ngroups, n);
         MDSM_REQUIRE(rt.ngroups <= 65535 && n <= 65535, "pre-pass: grid too large");
-        if (pre_smem > 48 * 1024) {
-            // only very wide groups need this; set per launch (per-device state)
-            switch (rt.G) {
-#define MDSM_PRE_ATTR(GG) case GG: \
-                MDSM_CUDA_TRY(cudaFuncSetAttribute(group_presum_f32_kernel<GG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pre_smem)); \
-                MDSM_CUDA_TRY(cudaFuncSetAttribute(group_presum_u8_kernel<GG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pre_smem)); break;
-                MDSM_PRE_ATTR(1) MDSM_PRE_ATTR(2) MDSM_PRE_ATTR(3) MDSM_PRE_ATTR(4) MDSM_PRE_ATTR(5) MDSM_PRE_ATTR(6) MDSM_PRE_ATTR(7) MDSM_PRE_ATTR(8)
-#undef MDSM_PRE_ATTR
-            }
-        }
+        cudaError_t pe;
         switch (rt.G) {
-            case 1: launch_presum<1>(f32, pa, grid, pre_smem, st); break;
-            case 2: launch_presum<2>(f32, pa, grid, pre_smem, st); break;
-            case 3: launch_presum<3>(f32, pa, grid, pre_smem, st); break;
-            case 4: launch_presum<4>(f32, pa, grid, pre_smem, st); break;
-            case 5: launch_presum<5>(f32, pa, grid, pre_smem, st); break;
-            case 6: launch_presum<6>(f32, pa, grid, pre_smem, st); break;
-            case 7: launch_presum<7>(f32, pa, grid, pre_smem, st); break;
-            default: launch_presum<8>(f32, pa, grid, pre_smem, st); break;
+            case 1: pe = launch_presum<1>(dtype, pa, grid, pre_smem, st); break;
+            case 2: pe = launch_presum<2>(dtype, pa, grid, pre_smem, st); break;
+            case 3: pe = launch_presum<3>(dtype, pa, grid, pre_smem, st); break;
+            case 4: pe = launch_presum<4>(dtype, pa, grid, pre_smem, st); break;
+            case 5: pe = launch_presum<5>(dtype, pa, grid, pre_smem, st); break;
+            case 6: pe = launch_presum<6>(dtype, pa, grid, pre_smem, st); break;
+            case 7: pe = launch_presum<7>(dtype, pa, grid, pre_smem, st); break;
+            default: pe = launch_presum<8>(dtype, pa, grid, pre_smem, st); break;
         }
+        MDSM_CUDA_TRY(pe);
         MDSM_CUDA_TRY(cudaGetLastError());
         p->launches += 1;
 
@@ -1154,6 +1215,7 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
         a.nsamps = p->nsamps; a.nsamps_out = p->nsamps_out; a.ystride = rt.ystride;
         const int grid_main = (int)std::min<long long>(a.ntiles, p->sm_count);
         if (f32) rc = launch_rows<RowsTraits<kGeomRowsF32.D, kGeomRowsF32.T, kGeomRowsF32.NW, true>>(a, rt.smem_bytes, grid_main, st);
+        else if (w32) rc = launch_rows<RowsTraits<kGeomRowsF32.D, kGeomRowsF32.T, kGeomRowsF32.NW, true, true>>(a, rt.smem_bytes, grid_main, st);
         else rc = launch_rows<RowsTraits<kGeomRowsU16.D, kGeomRowsU16.T, kGeomRowsU16.NW, false>>(a, rt.smem_bytes, grid_main, st);
         }
         if (rc != MDSM_OK) return rc;

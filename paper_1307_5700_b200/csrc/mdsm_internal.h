@@ -83,11 +83,13 @@ struct mdsm_plan {
 
     int dedisp_kernel = 0;            // option "dedisp_kernel": 0 auto, 1 direct, 2 rows
     int group_size = 0;               // option "group_size": channels per pre-summed group, 0 = chosen by the cost model
-    RowsTables rows_f32, rows_u8;
+    // rows_f32: 32-bit rows (MDSM_F32 and, with integer adds, MDSM_U16); rows_u8 / rows_u4: packed 16-bit rows, flushed to the
+    // uint32 output every 256 / 4096 channels (what a 16-bit lane holds of 255s / 15s)
+    RowsTables rows_f32, rows_u8, rows_u4;
     TmemTables tmem_f32;
-    void *d_scratch_f32 = nullptr, *d_scratch_u8 = nullptr;     // pre-summed rows [slots][nyrows][ystride] (mdsm_plan_reserve)
-    int scratch_slots_f32 = 0, scratch_slots_u8 = 0;            // beams the scratch holds at a time
-    size_t scratch_bytes_f32 = 0, scratch_bytes_u8 = 0;
+    void *d_scratch[4] = {nullptr, nullptr, nullptr, nullptr};  // per dtype: pre-summed rows [slots][nyrows][ystride] (mdsm_plan_reserve)
+    int scratch_slots[4] = {0, 0, 0, 0};                        // beams the scratch holds at a time
+    size_t scratch_bytes[4] = {0, 0, 0, 0};
 
     // host pipeline workspace (allocated on first mdsm_pipeline_host)
     void *ws_in = nullptr; size_t ws_in_bytes = 0;
@@ -101,6 +103,12 @@ struct mdsm_plan {
 
     int64_t launches = 0;
 };
+
+inline const RowsTables &mdsm_rows_of(const mdsm_plan *p, int dtype)
+{
+    return dtype == MDSM_U8 ? p->rows_u8 : (dtype == MDSM_U4 ? p->rows_u4 : p->rows_f32);
+}
+inline bool mdsm_dtype_ok(int dtype) { return dtype >= MDSM_F32 && dtype <= MDSM_U4; }
 
 // stage launchers (each returns an MDSM_* status)
 int mdsm_launch_clip(mdsm_plan *p, void *d_in, int dtype, int beam0, int nb, int window, double k_chan,

@@ -35,7 +35,7 @@ extern "C" int mdsm_pipeline_host(mdsm_plan *p, const void *h_in, int dtype, int
         // scratch of the dedispersion kernel (no-op once reserved).  Beam groups on different streams may only run
         // side by side when every beam has its own scratch slot; otherwise the whole chain goes through one stream.
         if ((rc = mdsm_plan_reserve(p, dtype, 0))) return rc;
-        const int slots = dtype == MDSM_F32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
+        const int slots = p->scratch_slots[dtype];
         if (slots > 0 && slots < p->nbeams) nstreams = 1;
     }
     const size_t esize = dtype == MDSM_F32 ? 4 : 1;

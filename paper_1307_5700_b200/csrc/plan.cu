@@ -133,8 +133,7 @@ extern "C" void mdsm_plan_destroy(mdsm_plan *p)
     cudaFree(p->d_series_stats);
     cudaFree(p->ws_filt);
     mdsm_rows_free_tables(p);
-    cudaFree(p->d_scratch_f32);
-    cudaFree(p->d_scratch_u8);
+    for (int k = 0; k < 4; ++k) cudaFree(p->d_scratch[k]);
     cudaFree(p->ws_in);
     cudaFree(p->ws_out);
     cudaFree(p->ws_events);
@@ -157,11 +156,12 @@ extern "C" int mdsm_plan_get_delays(const mdsm_plan *p, int32_t *h_delays)
 
 static void drop_scratch(mdsm_plan *p)
 {
-    cudaFree(p->d_scratch_f32);
-    cudaFree(p->d_scratch_u8);
-    p->d_scratch_f32 = p->d_scratch_u8 = nullptr;
-    p->scratch_slots_f32 = p->scratch_slots_u8 = 0;
-    p->scratch_bytes_f32 = p->scratch_bytes_u8 = 0;
+    for (int k = 0; k < 4; ++k) {
+        cudaFree(p->d_scratch[k]);
+        p->d_scratch[k] = nullptr;
+        p->scratch_slots[k] = 0;
+        p->scratch_bytes[k] = 0;
+    }
 }
 
 extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value)
@@ -194,11 +194,12 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
     return MDSM_EINVAL;
 }
 
-static int check_common(const mdsm_plan *p, const void *ptr, int dtype, int beam0, int nb)
+static int check_common(const mdsm_plan *p, const void *ptr, int dtype, int beam0, int nb, bool dedisp_input = false)
 {
     MDSM_REQUIRE(p, "null plan");
     MDSM_REQUIRE(ptr, "null data pointer");
-    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
+    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8 || (dedisp_input && mdsm_dtype_ok(dtype)),
+                 dedisp_input ? "dtype must be MDSM_F32, MDSM_U8, MDSM_U16 or MDSM_U4" : "dtype must be MDSM_F32 or MDSM_U8");
     MDSM_REQUIRE(beam0 >= 0 && nb >= 1 && beam0 + nb <= p->nbeams, "beam range [%d, %d) outside [0, %d)", beam0,
                  beam0 + nb, p->nbeams);
     int dev = -1;
@@ -234,15 +235,17 @@ extern "C" int mdsm_bandpass_clip(mdsm_plan *p, float *d_in, int beam0, int nb, 
 extern "C" int mdsm_dedisperse(mdsm_plan *p, const void *d_in, int dtype, int beam0, int nb, void *d_out,
                                void *cuda_stream)
 {
-    int rc = check_common(p, d_in, dtype, beam0, nb);
+    int rc = check_common(p, d_in, dtype, beam0, nb, true);
     if (rc) return rc;
     MDSM_REQUIRE(d_out, "null output pointer");
-    const RowsTables &rt = dtype == MDSM_F32 ? p->rows_f32 : p->rows_u8;
+    MDSM_REQUIRE(dtype != MDSM_U4 || p->nsamps % 2 == 0, "MDSM_U4 needs an even nsamps (two samples per byte)");
+    MDSM_REQUIRE(dtype != MDSM_U16 || (double)p->nchans * 65535.0 < 4294967296.0, "MDSM_U16: nchans * 65535 must fit 32 bits");
+    const RowsTables &rt = mdsm_rows_of(p, dtype);
     if (p->dedisp_kernel == 1 || (p->dedisp_kernel == 0 && !rt.ok))
         return mdsm_launch_dedisperse_direct(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
     MDSM_REQUIRE(rt.ok, "the pre-summed-rows kernel has no tables for this plan (see mdsm_plan_kernel_info)");
     MDSM_REQUIRE(p->dedisp_kernel != 3 || (dtype == MDSM_F32 && p->tmem_f32.ok), "the TMEM variant has no tables for this plan / dtype");
-    MDSM_REQUIRE(dtype == MDSM_F32 ? p->d_scratch_f32 != nullptr : p->d_scratch_u8 != nullptr,
+    MDSM_REQUIRE(p->d_scratch[dtype] != nullptr,
                  "dedispersion scratch not reserved: call mdsm_plan_reserve(plan, dtype, 0) once before mdsm_dedisperse");
     return mdsm_launch_dedisperse_rows(p, d_in, dtype, beam0, nb, d_out, (cudaStream_t)cuda_stream);
 }
@@ -250,14 +253,13 @@ extern "C" int mdsm_dedisperse(mdsm_plan *p, const void *d_in, int dtype, int be
 extern "C" int mdsm_plan_reserve(mdsm_plan *p, int dtype, int64_t max_bytes)
 {
     MDSM_REQUIRE(p, "null plan");
-    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
+    MDSM_REQUIRE(mdsm_dtype_ok(dtype), "dtype must be MDSM_F32, MDSM_U8, MDSM_U16 or MDSM_U4");
     MDSM_REQUIRE(max_bytes >= 0, "max_bytes must be >= 0 (0 = default)");
-    const bool f32 = dtype == MDSM_F32;
     const size_t per_beam = mdsm_rows_scratch_bytes_per_beam(p, dtype);
     if (per_beam == 0) return MDSM_OK;                       // this plan runs the direct kernel: nothing to reserve
-    void *&scratch = f32 ? p->d_scratch_f32 : p->d_scratch_u8;
-    int &slots = f32 ? p->scratch_slots_f32 : p->scratch_slots_u8;
-    size_t &bytes = f32 ? p->scratch_bytes_f32 : p->scratch_bytes_u8;
+    void *&scratch = p->d_scratch[dtype];
+    int &slots = p->scratch_slots[dtype];
+    size_t &bytes = p->scratch_bytes[dtype];
     size_t limit = (size_t)max_bytes;
     if (limit == 0) {
         size_t free_b = 0, total_b = 0;
@@ -288,9 +290,9 @@ extern "C" int mdsm_plan_reserve(mdsm_plan *p, int dtype, int64_t max_bytes)
 extern "C" int mdsm_plan_kernel_info(const mdsm_plan *p, int dtype, char *buf, int64_t buflen)
 {
     MDSM_REQUIRE(p && buf && buflen > 0, "null argument");
-    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "dtype must be MDSM_F32 or MDSM_U8");
+    MDSM_REQUIRE(mdsm_dtype_ok(dtype), "dtype must be MDSM_F32, MDSM_U8, MDSM_U16 or MDSM_U4");
     const bool f32 = dtype == MDSM_F32;
-    const RowsTables &rt = f32 ? p->rows_f32 : p->rows_u8;
+    const RowsTables &rt = mdsm_rows_of(p, dtype);
     const bool rows = p->dedisp_kernel != 1 && rt.ok;
     if (!rows) {
         snprintf(buf, (size_t)buflen, "kernel=direct reason=%s", p->dedisp_kernel == 1 ? "option" : "no_tables");
@@ -303,13 +305,13 @@ extern "C" int mdsm_plan_kernel_info(const mdsm_plan *p, int dtype, char *buf, i
                  "kernel=rows operands=tmem group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%.2f tmem_cols_per_group=%.1f "
                  "row_slots=%d row_pitch=%d stages=%d smem_bytes=%zu nyrows=%d scratch_slots=%d scratch_bytes=%zu",
                  rt.G, tt.DB, tt.span, tt.groups_per_slab, tt.cols_per_group, tt.CS, tt.pitch, tt.stages, tt.smem_bytes, rt.nyrows,
-                 p->scratch_slots_f32, p->scratch_bytes_f32);
+                 p->scratch_slots[dtype], p->scratch_bytes[dtype]);
     else
     snprintf(buf, (size_t)buflen,
              "kernel=rows operands=smem group_size=%d dms_per_block=%d tile_samples=%d groups_per_slab=%d row_slots=%d row_pitch=%d stages=%d "
              "smem_bytes=%zu nyrows=%d rows_per_block=%.0f scratch_slots=%d scratch_bytes=%zu",
              rt.G, rt.DB, rt.stride, rt.Q, rt.CS, rt.pitch, rt.stages, rt.smem_bytes, rt.nyrows, rt.rows_per_block,
-             f32 ? p->scratch_slots_f32 : p->scratch_slots_u8, f32 ? p->scratch_bytes_f32 : p->scratch_bytes_u8);
+             p->scratch_slots[dtype], p->scratch_bytes[dtype]);
     return 1;
 }
 

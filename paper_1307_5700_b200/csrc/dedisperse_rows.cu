@@ -473,23 +473,24 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
 // Tensor memory (TMEM, 128 lanes x 512 columns x 32 bit per SM) has its own read path into the register file
 // (tcgen05.ld), measured at ~3x that rate with the adds in the loop, and -- unlike registers -- its COLUMN address is
 // a run-time value.  So the operand window moves there:
-//   * TMEM lane l of a quadrant holds the samples  s0 + P l + [0, P + S)  of a staged y row in consecutive columns
-//     (P = outputs per lane and DM, S = spread of the window starts of the DMs that use the row);
+//   * TMEM lane l of a quadrant holds the samples  s0 + P l + [0, 16 + S)  of a staged y row in consecutive columns
+//     (P = 15 outputs per lane and DM, S = spread of the window starts of the DMs that use the row);
 //   * a consumer thread (lane l) owns the P consecutive outputs  tile_t0 - sigma_d + P l + [0, P)  of each of its D DMs
-//     and fetches, per (DM, group), P consecutive columns at the DM's own column offset: one tcgen05.ld.32x32b.x16 per
+//     and fetches, per (DM, group), 16 consecutive columns at the DM's own column offset: one tcgen05.ld.32x32b.x16 per
 //     15 adds, no alignment cases, no shared-memory traffic;
-//   * a STAGER warp per quadrant (TMEM lanes are only reachable from the warps w with w % 4 == quadrant) copies each
-//     row the quadrant's 4 D DMs use from the TMA-filled shared-memory stage into TMEM: conflict-free 32-bit loads
-//     (P is odd) + tcgen05.st.  A staged word then serves every DM of the quadrant that uses the row, so the
-//     shared-memory pipe carries ~0.5 words per add instead of 1.
-// Warps: 16 consumers (quadrant = w & 3, D DMs each), 4 stagers (w = 16..19), 1 TMA producer (w = 20); the two non-consumer
-// warpgroups hand most of their registers to the consumers (setmaxnreg).
-// Rings: shared-memory stages (producer -> stagers), two TMEM stages of 256 columns (stager -> the quadrant's consumers).
-constexpr int kTmWarps = 24;         // 16 consumers + 4 stagers + the producer's warpgroup (3 of its warps idle)
-constexpr int kTmProducer = 20;
-constexpr int kTmCols = 256;          // TMEM columns per stage (two stages)
+//   * the rows get into TMEM through the consumer warps themselves: TMEM lanes are only reachable from the warps w with
+//     w % 4 == quadrant, so the 4 warps of a quadrant share the copy of the rows their 16 DMs use, 16 columns at a time
+//     (conflict-free 32-bit shared-memory loads because P is odd, then tcgen05.st).  A staged word serves every DM of
+//     the quadrant that uses the row, so the shared-memory pipe carries ~0.5 words per add instead of 1.
+// Warps: 16 consumers (quadrant = w & 3, D DMs each) and 1 TMA producer (w = 16; its warpgroup hands registers to the
+// consumers with setmaxnreg).  Rings: shared-memory stages (producer -> consumers' staging half), two TMEM buffers of 256
+// columns per quadrant (staging half -> adding half of the same four warps, one slab ahead).
+constexpr int kTmWarps = 20;          // 16 consumers + the producer's warpgroup (3 of its warps idle)
+constexpr int kTmProducer = 16;
+constexpr int kTmCols = 256;          // TMEM columns per buffer (two buffers)
 constexpr int kTmQMax = 4;            // most groups per slab
-constexpr int kTmRQMax = 16;          // most staged rows per quadrant and slab
+constexpr int kTmCQMax = 32;          // most 16-column chunks per quadrant and slab
+constexpr int kTmEnt = 20;            // words of a warp's entry copy (D * kTmQMax entries + the group count, padded)
 
 struct TmemArgs {
     const float *y;
@@ -528,18 +529,40 @@ __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sy
 __device__ __forceinline__ void tm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
+// walks the slabs of the tiles a CTA owns, in order
+struct TmSlabIter {
+    long long tile;
+    int blk, nslab, slab;
+    __device__ __forceinline__ void init(const TmemArgs &a)
+    {
+        tile = blockIdx.x;
+        slab = 0;
+        load(a);
+    }
+    __device__ __forceinline__ void load(const TmemArgs &a)
+    {
+        if (tile < a.ntiles) { blk = (int)(tile % a.nblk); nslab = a.nslab[blk]; }
+    }
+    __device__ __forceinline__ bool valid(const TmemArgs &a) const { return tile < a.ntiles; }
+    __device__ __forceinline__ void advance(const TmemArgs &a)
+    {
+        if (++slab == nslab) { slab = 0; tile += gridDim.x; load(a); }
+    }
+};
+
 template <int D, int P>
 __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const TmemArgs a)
 {
     static_assert(P % 2 == 1 && P <= 16, "P must be odd (conflict-free staging) and fit one x16 load");
-    constexpr int DQ = 4 * D, DB = 16 * D, TENT = DQ * kTmQMax + 4;
+    static_assert(D * kTmQMax + 1 <= kTmEnt, "entry copy too small");
+    constexpr int DQ = 4 * D, DB = 16 * D;
     extern __shared__ __align__(128) unsigned char smem[];
     const int stages = a.stages;
     const uint32_t row_bytes = (uint32_t)a.pitch * 4u;
     const uint32_t tab_bytes = (uint32_t)a.tabw * 4u;
     const uint32_t stage_bytes = (a.CS * row_bytes + tab_bytes + 127u) & ~127u;
-    uint32_t *tent = reinterpret_cast<uint32_t *>(smem + (size_t)stages * stage_bytes);       // [2][4][TENT]
-    uint64_t *full = reinterpret_cast<uint64_t *>(tent + 2 * 4 * TENT);
+    uint32_t *tent = reinterpret_cast<uint32_t *>(smem + (size_t)stages * stage_bytes);       // [2][16][kTmEnt]
+    uint64_t *full = reinterpret_cast<uint64_t *>(tent + 2 * 16 * kTmEnt);
     uint64_t *empty = full + stages;
     uint64_t *tfull = empty + stages;          // [2][4]
     uint64_t *tempty = tfull + 8;              // [2][4]
@@ -551,10 +574,10 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 32);
-            mbar_init(&empty[s], 4);
+            mbar_init(&empty[s], 16);
         }
         for (int s = 0; s < 8; ++s) {
-            mbar_init(&tfull[s], 1);
+            mbar_init(&tfull[s], 4);
             mbar_init(&tempty[s], 4);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -567,12 +590,9 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
     __syncthreads();
     tm_fence_after();
     const uint32_t tbase = *tbase_slot;
-    if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-    else asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
-
-    if (warp > kTmProducer) {
-        // idle warps of the producer's warpgroup
-    } else if (warp == kTmProducer) {
+    if (warp >= kTmProducer) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+      if (warp == kTmProducer) {
         // ===== TMA producer: lane r copies row r of every slab, lane 0 also the slab's table slice =====
         int st = 0;
         uint32_t ph = 1;
@@ -608,73 +628,72 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
                 if (++st == stages) { st = 0; ph ^= 1; first_lap = false; }
             }
         }
-    } else if (warp >= 16) {
-        // ===== stager of quadrant q: shared-memory stage -> TMEM stage =====
-        const int q = warp & 3;
-        const uint32_t tq = tbase + ((uint32_t)(q * 32) << 16);
-        int st = 0, ts = 0;
-        uint32_t ph = 0, tph = 1;
-        bool tfirst = true;
-        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-            const int nslab = a.nslab[(int)(tile % a.nblk)];
-            for (int slab = 0; slab < nslab; ++slab) {
-                mbar_wait(&full[st], ph);
-                const unsigned char *sbase = smem + (size_t)st * stage_bytes;
-                const uint32_t *tab = reinterpret_cast<const uint32_t *>(sbase + a.CS * row_bytes);
-                const int nr = (int)tab[q];
-                if (!tfirst) mbar_wait(&tempty[ts * 4 + q], tph);
-                tm_fence_after();
-                const float *rows = reinterpret_cast<const float *>(sbase) + P * lane;
-                const uint32_t tstage = tq + ts * kTmCols;
-#pragma unroll 1
-                for (int r = 0; r < nr; ++r) {
-                    const uint32_t soff = tab[8 + (q * kTmRQMax + r) * 2], w1 = tab[8 + (q * kTmRQMax + r) * 2 + 1];
-                    const float *src = rows + soff;
-                    const uint32_t tcol = tstage + (w1 & 0xffffu);
-                    const int n8 = (int)(w1 >> 16);
-                    int k = 0;
-#pragma unroll 1
-                    for (; k + 2 <= n8; k += 2) {                 // 16 columns per round: all the loads are in flight together
-                        uint32_t v[16];
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(src[8 * k + i]);
-                        tm_st16(tcol + 8 * k, v);
-                    }
-                    if (k < n8) {
-                        uint32_t v[8];
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) v[i] = __float_as_uint(src[8 * k + i]);
-                        tm_st8(tcol + 8 * k, v);
-                    }
-                }
-                // the quadrant's entries (TMEM column per (DM, group)) and the number of groups of this slab
-                uint32_t *te = tent + (ts * 4 + q) * TENT;
-                const uint32_t *ent = tab + 8 + 4 * kTmRQMax * 2 + q * DQ * kTmQMax;
-                for (int i = lane; i < DQ * kTmQMax; i += 32) te[i] = ent[i];
-                if (lane == 0) te[DQ * kTmQMax] = tab[4];
-                tm_wait_st();
-                tm_fence_before();
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(&tfull[ts * 4 + q]);
-                    mbar_arrive(&empty[st]);
-                }
-                if (++st == stages) { st = 0; ph ^= 1; }
-                if (++ts == 2) { ts = 0; tph ^= 1; tfirst = false; }
-            }
-        }
+      }
     } else {
-        // ===== consumers: warp (q, sub) owns the DMs q DQ + sub D + j of the block =====
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+        // ===== consumers: warp (q, sub) owns the DMs q DQ + sub D + j of the block; the four warps of a quadrant stage the
+        // quadrant's rows of slab n + 1 into TMEM buffer (n + 1) & 1, then add slab n out of buffer n & 1 =====
         const int q = warp & 3, sub = warp >> 2;
         const uint32_t tq = tbase + ((uint32_t)(q * 32) << 16);
-        int ts = 0;
-        uint32_t tph = 0;
-        for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-            const int blk = (int)(tile % a.nblk);
-            const long long rest = tile / a.nblk;
+        uint32_t *my_ent = tent + warp * kTmEnt;                 // + buffer * 16 * kTmEnt
+        TmSlabIter si, ci;
+        si.init(a);
+        ci.init(a);
+        uint32_t nstaged = 0, nadded = 0;                        // slabs staged / added so far by this warp
+        int sst = 0;                                             // shared-memory stage of the next slab to stage
+        uint32_t sph = 0;
+
+        auto stage_one = [&]() {
+            const int buf = nstaged & 1;
+            mbar_wait(&full[sst], sph);
+            if (nstaged >= 2) {                                  // the buffer's previous slab must have been added by all four warps
+                while (!mbar_try_wait(&tempty[buf * 4 + q], ((nstaged >> 1) - 1) & 1)) {}
+            }
+            tm_fence_after();
+            const unsigned char *sbase = smem + (size_t)sst * stage_bytes;
+            const uint32_t *tab = reinterpret_cast<const uint32_t *>(sbase + a.CS * row_bytes);
+            const int nch = (int)tab[q];
+            const float *rows = reinterpret_cast<const float *>(sbase) + P * lane;
+            const uint32_t tbuf = tq + buf * kTmCols;
+#pragma unroll 1
+            for (int j = sub; j < nch; j += 4) {
+                const uint32_t soff = tab[8 + (q * kTmCQMax + j) * 2], w1 = tab[8 + (q * kTmCQMax + j) * 2 + 1];
+                const float *src = rows + soff;
+                const uint32_t tcol = tbuf + (w1 & 0xffffu);
+                if (w1 >> 16) {                                  // 16 columns
+                    uint32_t v[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(src[i]);
+                    tm_st16(tcol, v);
+                } else {
+                    uint32_t v[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) v[i] = __float_as_uint(src[i]);
+                    tm_st8(tcol, v);
+                }
+            }
+            // this warp's entries (TMEM column per (DM, group)) and the number of groups of the slab
+            const uint32_t *ent = tab + 8 + 4 * kTmCQMax * 2 + (q * DQ + sub * D) * kTmQMax;
+            uint32_t *te = my_ent + buf * 16 * kTmEnt;
+            if (lane < D * kTmQMax) te[lane] = ent[lane];
+            if (lane == 31) te[D * kTmQMax] = tab[4];
+            tm_wait_st();
+            tm_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&tfull[buf * 4 + q]);
+                mbar_arrive(&empty[sst]);
+            }
+            if (++sst == stages) { sst = 0; sph ^= 1; }
+            ++nstaged;
+        };
+
+        if (si.valid(a)) { stage_one(); si.advance(a); }
+        while (ci.valid(a)) {
+            const long long rest = ci.tile / a.nblk;
             const int tt = (int)(rest % a.ntile_t), bb = (int)(rest / a.ntile_t);
             const long long tile_t0 = (long long)tt * a.span;
-            const int nslab = a.nslab[blk];
+            const int blk = ci.blk, nslab = ci.nslab;
             float acc[D][P];
 #pragma unroll
             for (int j = 0; j < D; ++j)
@@ -682,21 +701,22 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
                 for (int i = 0; i < P; ++i) acc[j][i] = 0.0f;
 #pragma unroll 1
             for (int slab = 0; slab < nslab; ++slab) {
-                while (!mbar_try_wait(&tfull[ts * 4 + q], tph)) __nanosleep(64);      // no hot spinning beside the stager
+                if (si.valid(a)) { stage_one(); si.advance(a); }
+                const int buf = nadded & 1;
+                while (!mbar_try_wait(&tfull[buf * 4 + q], (nadded >> 1) & 1)) {}
                 tm_fence_after();
-                const uint32_t *te = tent + (ts * 4 + q) * TENT;
-                const int nq = (int)te[DQ * kTmQMax];
-                const uint32_t *ents = te + sub * D * kTmQMax;
-                const uint32_t tstage = tq + ts * kTmCols;
+                const uint32_t *te = my_ent + buf * 16 * kTmEnt;
+                const int nq = (int)te[D * kTmQMax];
+                const uint32_t tbuf = tq + buf * kTmCols;
 #pragma unroll 1
                 for (int g = 0; g < nq; ++g) {
                     uint32_t e[D];
 #pragma unroll
-                    for (int j = 0; j < D; ++j) e[j] = ents[j * kTmQMax + g];
+                    for (int j = 0; j < D; ++j) e[j] = te[j * kTmQMax + g];
 #pragma unroll
                     for (int j = 0; j < D; ++j) {
                         uint32_t v[16];
-                        tm_ld16(tstage + e[j], v);
+                        tm_ld16(tbuf + e[j], v);
                         tm_wait_ld();
 #pragma unroll
                         for (int i = 0; i < P; ++i) acc[j][i] += __uint_as_float(v[i]);
@@ -704,8 +724,9 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
                 }
                 tm_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&tempty[ts * 4 + q]);
-                if (++ts == 2) { ts = 0; tph ^= 1; }
+                if (lane == 0) mbar_arrive(&tempty[buf * 4 + q]);
+                ++nadded;
+                ci.advance(a);
             }
             const int b = a.beam0 + bb;
 #pragma unroll
@@ -726,6 +747,7 @@ __global__ void __launch_bounds__(kTmWarps * 32, 1) dedisperse_tmem_kernel(const
     __syncthreads();
     if (warp == kTmProducer) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
 }
+
 
 // ------------------------------------------------------------------ host side: the plan-time tables
 struct RowsGeom { int D, T, NW; };
@@ -919,13 +941,13 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
     for (int dl = 0; dl < DB; ++dl) h.sigma[dl] = (int32_t)llround(0.5 * smax * dl);
     auto dly = [&](int d, int c) { return (long long)p->h_delay[(size_t)d * p->nchans + c]; };
     struct Use { int yrow; long long emin, emax; };
-    struct GroupUse { std::vector<Use> blk; std::vector<Use> quad[4]; int cols[4]; };
+    struct GroupUse { std::vector<Use> blk; std::vector<Use> quad[4]; int cols[4], chunks[4]; };
     auto add_use = [](std::vector<Use> &u, int yr, long long e) {
         auto it = std::find_if(u.begin(), u.end(), [&](const Use &x) { return x.yrow == yr; });
         if (it == u.end()) u.push_back({yr, e, e});
         else { it->emin = std::min(it->emin, e); it->emax = std::max(it->emax, e); }
     };
-    const int tabw = 8 + 4 * kTmRQMax * 2 + DB * kTmQMax;
+    const int tabw = 8 + 4 * kTmCQMax * 2 + DB * kTmQMax;
     std::vector<std::vector<GroupUse>> gu(nblk, std::vector<GroupUse>(ng));
     long long need_max = 0;
     for (int blk = 0; blk < nblk; ++blk)
@@ -939,9 +961,13 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
                 add_use(u.quad[dl / DQ], yr, e);
             }
             for (int q = 0; q < 4; ++q) {
-                u.cols[q] = 0;
-                for (const Use &x : u.quad[q]) u.cols[q] += (int)ceil_to(16 + (x.emax - x.emin), 8);   // the consumers load 16 columns
-                if (u.cols[q] > kTmCols || (int)u.quad[q].size() > kTmRQMax) return false;
+                u.cols[q] = u.chunks[q] = 0;
+                for (const Use &x : u.quad[q]) {
+                    const int c8 = (int)ceil_to(16 + (x.emax - x.emin), 8);      // the consumers load 16 columns
+                    u.cols[q] += c8;
+                    u.chunks[q] += (c8 + 15) / 16;                                // staged 16 columns at a time (+ one 8)
+                }
+                if (u.cols[q] > kTmCols || u.chunks[q] > kTmCQMax) return false;
             }
             if (u.blk.size() > 32) return false;
             for (const Use &x : u.blk) need_max = std::max(need_max, x.emax - floor_to(x.emin, al) + span);
@@ -960,10 +986,10 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
             while (g1 < ng && g1 - g0 < kTmQMax) {
                 const GroupUse &u = gu[blk][g1];
                 bool fits = rows + (int)u.blk.size() <= 32;
-                for (int q = 0; q < 4; ++q) fits = fits && cols[q] + u.cols[q] <= kTmCols && nrq[q] + (int)u.quad[q].size() <= kTmRQMax;
+                for (int q = 0; q < 4; ++q) fits = fits && cols[q] + u.cols[q] <= kTmCols && nrq[q] + u.chunks[q] <= kTmCQMax;
                 if (!fits) break;
                 rows += (int)u.blk.size();
-                for (int q = 0; q < 4; ++q) { cols[q] += u.cols[q]; nrq[q] += (int)u.quad[q].size(); cols_total += u.cols[q]; }
+                for (int q = 0; q < 4; ++q) { cols[q] += u.cols[q]; nrq[q] += u.chunks[q]; cols_total += u.cols[q]; }
                 ++g1;
             }
             if (g1 == g0) return false;
@@ -977,7 +1003,7 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
     }
     const int CS = cs_max;
     const size_t stage = (((size_t)CS * pitch * 4 + (size_t)tabw * 4) + 127) & ~(size_t)127;
-    const size_t fixed = (size_t)2 * 4 * (DQ * kTmQMax + 4) * 4 + 320;      // entry copies, barriers, TMEM base slot
+    const size_t fixed = (size_t)2 * 16 * kTmEnt * 4 + 320;                  // entry copies, barriers, TMEM base slot
     const int stages = (int)std::min<size_t>(8, (kSmemBudget - fixed - 64) / stage);
     if (stages < 2) return false;
     h.rowdesc.assign((size_t)nblk * nslab_max * CS, make_int4(-1, 0, 0, 0));
@@ -1004,12 +1030,18 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
                         size_t kb = 0;
                         while (u.blk[kb].yrow != x.yrow) ++kb;
                         const long long rs = floor_to(u.blk[kb].emin, al);
-                        const int n8 = (int)ceil_to(16 + (x.emax - x.emin), 8) / 8;
-                        const int slot = nrq[q]++;
-                        tab[8 + (q * kTmRQMax + slot) * 2] = (uint32_t)((long long)(r + kb) * pitch + (x.emin - rs));
-                        tab[8 + (q * kTmRQMax + slot) * 2 + 1] = (uint32_t)tcol[q] | ((uint32_t)n8 << 16);
+                        int n8 = (int)ceil_to(16 + (x.emax - x.emin), 8) / 8;
                         col_of[k] = tcol[q];
-                        tcol[q] += 8 * n8;
+                        uint32_t soff = (uint32_t)((long long)(r + kb) * pitch + (x.emin - rs));
+                        while (n8 > 0) {                                          // chunks of 16 columns, then one of 8
+                            const int c = n8 >= 2 ? 2 : 1;
+                            const int slot = nrq[q]++;
+                            tab[8 + (q * kTmCQMax + slot) * 2] = soff;
+                            tab[8 + (q * kTmCQMax + slot) * 2 + 1] = (uint32_t)tcol[q] | ((uint32_t)(c - 1) << 16);
+                            soff += 8 * c;
+                            tcol[q] += 8 * c;
+                            n8 -= c;
+                        }
                     }
                     for (int dq = 0; dq < DQ; ++dq) {
                         const int dl = q * DQ + dq;
@@ -1018,7 +1050,7 @@ static bool build_tmem_tables(const mdsm_plan *p, const GroupRows &gr, TmemTable
                         size_t k = 0;
                         while (u.quad[q][k].yrow != yr) ++k;
                         const long long e = dly(d, gi * G) - h.sigma[dle];
-                        tab[8 + 4 * kTmRQMax * 2 + (size_t)dl * kTmQMax + qi] = (uint32_t)(col_of[k] + (e - u.quad[q][k].emin));
+                        tab[8 + 4 * kTmCQMax * 2 + (size_t)dl * kTmQMax + qi] = (uint32_t)(col_of[k] + (e - u.quad[q][k].emin));
                     }
                 }
                 r += (int)u.blk.size();

@@ -72,6 +72,8 @@ const char *mdsm_last_error(void);
  *      main kernel, slower than 2 today -- DESIGN.md section 6.1) or MDSM_EINVAL.
  *  "group_size": channels per pre-summed group, 1..8, or 0 (default) = the plan's cost model picks it.  Changing it
  *      rebuilds the tables and DROPS the scratch reservation (call mdsm_plan_reserve again).
+ *  "detect_two_pass": 0 (default) = mdsm_detect is ONE launch (a CTA per series: statistics from HBM, thresholding of the same row
+ *      out of L2); 1 = the two-launch form (statistics kernel, then a grid over (time, series)), kept for comparison.
  *  "post_median_window" (0 = off, else odd <= 33) and "post_detrend" (0/1): mdsm_pipeline_host runs
  *      mdsm_median_filter / mdsm_detrend on the fp32 series between dedispersion and detection (ignored for uint8).
  * Unknown key/value -> MDSM_EINVAL. */

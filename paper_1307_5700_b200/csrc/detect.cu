@@ -86,21 +86,12 @@ series_stats_kernel(const T *__restrict__ out, int beam0, int ndms, long long ns
     }
 }
 
+// Thresholds the four samples t0 .. t0+3 of one series x (n valid samples) and appends the events; called by whole warps.
 template <typename T>
-__global__ void __launch_bounds__(kThreads)
-threshold_emit_kernel(const T *__restrict__ out, int beam0, int ndms, long long nsamps, long long n,
-                      const double *__restrict__ stats, double thr, mdsm_event *__restrict__ events,
-                      long long max_events, unsigned long long *__restrict__ count)
+__device__ __forceinline__ void threshold_emit4(const T *__restrict__ x, long long n, long long t0, int b, int d, double mean,
+                                                double rms, double thr, double cut, mdsm_event *__restrict__ events,
+                                                long long max_events, unsigned long long *__restrict__ count)
 {
-    const int d = blockIdx.y, b = beam0 + blockIdx.z;
-    const double mean = stats[((size_t)b * ndms + d) * 2];
-    const double rms = stats[((size_t)b * ndms + d) * 2 + 1];
-    if (rms == 0.0) return;                          // whole CTA: uniform
-    // snr > thr  =>  x - mean > thr*rms*(1 - 2^-40): cheap conservative pre-filter (thr*rms >= 0);
-    // for negative thresholds every sample is a candidate.
-    const double cut = thr > 0.0 ? thr * rms * (1.0 - 9.094947017729282e-13) : -1.7976931348623157e308;
-    const T *x = out + ((size_t)b * ndms + d) * (size_t)nsamps;
-    const long long t0 = ((long long)blockIdx.x * kThreads + threadIdx.x) * 4;
     T v[4];
     if (t0 + 3 < n && ((uintptr_t)x % 16 == 0)) {
         const uint4 u = *reinterpret_cast<const uint4 *>(x + t0);
@@ -162,18 +153,147 @@ threshold_emit_kernel(const T *__restrict__ out, int beam0, int ndms, long long 
 }
 
 template <typename T>
+__global__ void __launch_bounds__(kThreads)
+threshold_emit_kernel(const T *__restrict__ out, int beam0, int ndms, long long nsamps, long long n,
+                      const double *__restrict__ stats, double thr, mdsm_event *__restrict__ events,
+                      long long max_events, unsigned long long *__restrict__ count)
+{
+    const int d = blockIdx.y, b = beam0 + blockIdx.z;
+    const double mean = stats[((size_t)b * ndms + d) * 2];
+    const double rms = stats[((size_t)b * ndms + d) * 2 + 1];
+    if (rms == 0.0) return;                          // whole CTA: uniform
+    // snr > thr  =>  x - mean > thr*rms*(1 - 2^-40): cheap conservative pre-filter (thr*rms >= 0);
+    // for negative thresholds every sample is a candidate.
+    const double cut = thr > 0.0 ? thr * rms * (1.0 - 9.094947017729282e-13) : -1.7976931348623157e308;
+    const T *x = out + ((size_t)b * ndms + d) * (size_t)nsamps;
+    const long long t0 = ((long long)blockIdx.x * kThreads + threadIdx.x) * 4;
+    threshold_emit4<T>(x, n, t0, b, d, mean, rms, thr, cut, events, max_events, count);
+}
+
+// a5 + a6 in ONE launch and ONE read of `out`: a CTA of 256 threads owns a series (several CTAs per SM overlap their passes).  Pass 1 (from HBM) reduces S and Q and
+// records the maximum of every 128-sample chunk (what one warp loads per step) in shared memory; once mean and rms are
+// known, pass 2 looks at the chunk maxima only and re-reads (from L2) just the chunks that can hold an event:
+// snr > thr  =>  x > mean + thr*rms*(1 - 2^-40), a bound rounded down in the element type.
+constexpr int kFusedThreads = 256;
+template <typename T>
+__global__ void __launch_bounds__(kFusedThreads)
+detect_fused_kernel(const T *__restrict__ out, int beam0, int ndms, long long nsamps, long long n, double *__restrict__ stats,
+                    double thr, mdsm_event *__restrict__ events, long long max_events, unsigned long long *__restrict__ count)
+{
+    using A = typename SAcc<T>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *cmax = reinterpret_cast<T *>(smem_raw);                    // [ceil(n4 / 32)] chunk maxima
+    const int d = blockIdx.x, b = beam0 + blockIdx.y;
+    const T *x = out + ((size_t)b * ndms + d) * (size_t)nsamps;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    A S = 0, Q = 0;
+    const bool vec = ((uintptr_t)x % 16 == 0);
+    const long long n4 = vec ? n / 4 : 0;
+    const uint4 *xv = reinterpret_cast<const uint4 *>(x);
+    constexpr int U = 4;                                                  // independent 128-bit loads in flight per thread
+    const T lowest = kIsFloat<T> ? (T)(-3.402823466e38f) : (T)0;
+    for (long long base = 0; base < n4; base += (long long)U * kFusedThreads) {
+        uint4 v[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kFusedThreads + threadIdx.x;
+            v[u] = i < n4 ? xv[i] : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kFusedThreads + threadIdx.x;
+            T m = lowest;
+            if (i < n4) {
+                const unsigned w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const T t = as_elem<T>(w[k]);
+                    const A e = (A)t;
+                    S += e;
+                    Q += e * e;
+                    m = t > m ? t : m;
+                }
+            }
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) {
+                const T other = __shfl_xor_sync(0xffffffffu, m, o);
+                m = other > m ? other : m;
+            }
+            const long long c = ((base + (long long)u * kFusedThreads) >> 5) + warp;
+            if (lane == 0 && c * 32 < n4) cmax[c] = m;
+        }
+    }
+    for (long long i = n4 * 4 + threadIdx.x; i < n; i += kFusedThreads) {
+        A e = (A)x[i];
+        S += e;
+        Q += e * e;
+    }
+    __shared__ A red[2][kFusedThreads / 32];
+    __shared__ double s_stats[2];
+    S = wsum(S);
+    Q = wsum(Q);
+    if (lane == 0) { red[0][warp] = S; red[1][warp] = Q; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        A s = 0, q = 0;
+        for (int i = 0; i < kFusedThreads / 32; ++i) { s += red[0][i]; q += red[1][i]; }
+        const double dn = (double)n;
+        const double mean = __ddiv_rn((double)s, dn);
+        double var = __dsub_rn(__ddiv_rn((double)q, dn), __dmul_rn(mean, mean));
+        if (var < 0.0) var = 0.0;
+        double *o = stats + ((size_t)b * ndms + d) * 2;
+        o[0] = s_stats[0] = mean;
+        o[1] = s_stats[1] = __dsqrt_rn(var);
+    }
+    __syncthreads();
+    const double mean = s_stats[0], rms = s_stats[1];
+    if (rms == 0.0) return;
+    const double cut = thr > 0.0 ? thr * rms * (1.0 - 9.094947017729282e-13) : -1.7976931348623157e308;
+    // the same conservative bound threshold_emit4 applies per sample, here per chunk maximum
+    const double bound = mean + cut;
+    const double slack = bound - (fabs(bound) * 1e-12 + 1e-300);
+    bool all = false;
+    T cb;
+    if (kIsFloat<T>) {
+        cb = (T)__double2float_rd(slack);
+        all = !(slack > -3.0e38);
+    } else {
+        const double fl = floor(slack);
+        all = fl < 0.0;
+        cb = (T)(all ? 0u : (fl >= 4294967295.0 ? 0xffffffffu : (uint32_t)fl));
+    }
+    const long long nchunks = (n4 + 31) / 32;
+    for (long long c = warp; c < nchunks; c += kFusedThreads / 32)
+        if (all || cmax[c] > cb) threshold_emit4<T>(x, n, (c * 32 + lane) * 4, b, d, mean, rms, thr, cut, events, max_events, count);
+    // what the vector loop did not cover (an unaligned row: everything; else the last n % 4 samples)
+    for (long long t0 = n4 * 4 + (long long)threadIdx.x * 4; t0 - (long long)lane * 4 < n; t0 += (long long)kFusedThreads * 4)
+        threshold_emit4<T>(x, n, t0, b, d, mean, rms, thr, cut, events, max_events, count);
+}
+
+template <typename T>
 int launch_detect_t(mdsm_plan *p, const T *out, int beam0, int nb, double thr, mdsm_event *ev, long long max_events,
                     unsigned long long *count, cudaStream_t st)
 {
     MDSM_REQUIRE(p->ndms <= 65535 && nb <= 65535, "ndms and nb must be <= 65535");
     dim3 g1(p->ndms, nb);
-    series_stats_kernel<T><<<g1, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats);
+    if (p->detect_two_pass) {
+        // the two-launch form (statistics, then a grid over (time, series)): kept for comparison (option "detect_two_pass")
+        series_stats_kernel<T><<<g1, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats);
+        MDSM_CUDA_TRY(cudaGetLastError());
+        dim3 g2((unsigned)((p->nsamps_out + kThreads * 4 - 1) / (kThreads * 4)), p->ndms, nb);
+        threshold_emit_kernel<T><<<g2, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats,
+                                                          thr, ev, max_events, count);
+        MDSM_CUDA_TRY(cudaGetLastError());
+        p->launches += 2;
+        return MDSM_OK;
+    }
+    const size_t fsmem = (size_t)((p->nsamps_out / 4 + 31) / 32 + 1) * sizeof(T);
+    MDSM_REQUIRE(fsmem <= 160 * 1024, "series too long for the fused detection kernel (set option detect_two_pass)");
+    if (fsmem > 48 * 1024) MDSM_CUDA_TRY(cudaFuncSetAttribute(detect_fused_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
+    detect_fused_kernel<T><<<g1, kFusedThreads, fsmem, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats, thr, ev,
+                                                        max_events, count);
     MDSM_CUDA_TRY(cudaGetLastError());
-    dim3 g2((unsigned)((p->nsamps_out + kThreads * 4 - 1) / (kThreads * 4)), p->ndms, nb);
-    threshold_emit_kernel<T><<<g2, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats,
-                                                      thr, ev, max_events, count);
-    MDSM_CUDA_TRY(cudaGetLastError());
-    p->launches += 2;
+    p->launches += 1;
     return MDSM_OK;
 }
 

@@ -81,6 +81,7 @@ struct mdsm_plan {
     // detect scratch
     double *d_series_stats = nullptr; // [nbeams][ndms][2] = mean, rms
 
+    int detect_two_pass = 0;          // option "detect_two_pass": 1 = statistics and thresholding as two launches (comparison)
     int dedisp_kernel = 0;            // option "dedisp_kernel": 0 auto, 1 direct, 2 rows
     int group_size = 0;               // option "group_size": channels per pre-summed group, 0 = chosen by the cost model
     // rows_f32: 32-bit rows (MDSM_F32 and, with integer adds, MDSM_U16); rows_u8 / rows_u4: packed 16-bit rows, flushed to the

@@ -185,6 +185,11 @@ extern "C" int mdsm_plan_set_option(mdsm_plan *p, const char *key, int64_t value
         p->post_median_window = (int)value;
         return MDSM_OK;
     }
+    if (strcmp(key, "detect_two_pass") == 0) {
+        MDSM_REQUIRE(value == 0 || value == 1, "detect_two_pass must be 0 or 1");
+        p->detect_two_pass = (int)value;
+        return MDSM_OK;
+    }
     if (strcmp(key, "post_detrend") == 0) {
         MDSM_REQUIRE(value == 0 || value == 1, "post_detrend must be 0 or 1");
         p->post_detrend = (int)value;

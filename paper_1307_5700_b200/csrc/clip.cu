@@ -106,7 +106,8 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
 
     Acc S = 0, Q = 0;
     if (MODE == 0) {
-        const int g = window / V;
+        const int g = window / V;                              // a power of two <= 32 in this mode
+        const int gshift = __ffs(g) - 1;
         const long long nvec = nsamps / V;
         const typename E::Vec *vrow = reinterpret_cast<const typename E::Vec *>(row);
         for (long long base = 0; base < nvec; base += kThreads) {
@@ -116,7 +117,7 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
             S += s;
             Q += q;
             for (int m = 1; m < g; m <<= 1) s += shfl_xor<Acc>(s, m);
-            if (i < nvec && (lane & (g - 1)) == 0) csum[i / g] = (double)s;
+            if (i < nvec && (lane & (g - 1)) == 0) csum[i >> gshift] = (double)s;      // no 64-bit division in the loop
         }
     } else if (MODE == 1) {
         const int g = window / V;

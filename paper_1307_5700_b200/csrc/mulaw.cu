@@ -41,7 +41,9 @@ __device__ __forceinline__ unsigned code_of(float x, double xmax, double mu, dou
     const float vf = mu_f >= 1.0f ? 255.0f * (__log2f(1.0f + mu_f * __fdividef(x, xmax_f)) * inv_den_f)
                                   : 255.0f * (log1pf(mu_f * (x / xmax_f)) * inv_den_f);
     const float fr = vf - floorf(vf);
-    if (fabsf(fr - 0.5f) >= 1e-3f) return (unsigned)floorf(vf + 0.5f);
+    // guard band: 1e-3 for log1pf; 2.5e-4 for the hardware log2 with mu >= 1 (its error in vf is below 5e-5: 2 ulp of a
+    // result <= log2(1 + mu), scaled by 255 / log2(1 + mu))
+    if (fabsf(fr - 0.5f) >= (mu_f >= 1.0f ? 2.5e-4f : 1e-3f)) return (unsigned)floorf(vf + 0.5f);
     const double v = 255.0 * (log1p(mu * ((double)x / xmax)) * inv_den);
     return (unsigned)floor(v + 0.5);
 }

@@ -13,7 +13,7 @@
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kPer = 4;                         // outputs per thread
+constexpr int kPer = 8;                         // outputs per thread (that many independent loads in flight while staging)
 constexpr int kTile = kThreads * kPer;          // outputs per CTA
 constexpr int kMaxHalf = 16;                    // window <= 33
 
@@ -106,14 +106,25 @@ detrend_kernel(float *__restrict__ series, int beam0, int ndms, long long nsamps
     // pass 1 (HBM): regression sums and the sum of squares; the residual variance follows algebraically,
     //   sum r^2 = sum (y - mean)^2 - slope^2 * sum (t - tbar)^2   (fp64: cancellation ~1e-14 relative)
     double sy = 0.0, syy = 0.0, sty = 0.0;
-    for (long long i = threadIdx.x; i < n4; i += kThreads) {
-        const float4 q = reinterpret_cast<const float4 *>(x)[i];
-        const double v[4] = {(double)q.x, (double)q.y, (double)q.z, (double)q.w};
+    constexpr int U = 4;                                    // independent 128-bit loads in flight per thread
+    for (long long base = 0; base < n4; base += (long long)U * kThreads) {
+        float4 q[U];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            sy += v[k];
-            syy += v[k] * v[k];
-            sty += ((double)(4 * i + k) - tbar) * v[k];
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kThreads + threadIdx.x;
+            q[u] = i < n4 ? reinterpret_cast<const float4 *>(x)[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kThreads + threadIdx.x;
+            if (i >= n4) continue;
+            const double v[4] = {(double)q[u].x, (double)q[u].y, (double)q[u].z, (double)q[u].w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                sy += v[k];
+                syy += v[k] * v[k];
+                sty += ((double)(4 * i + k) - tbar) * v[k];
+            }
         }
     }
     for (long long t = n4 * 4 + threadIdx.x; t < n; t += kThreads) {
@@ -135,14 +146,25 @@ detrend_kernel(float *__restrict__ series, int beam0, int ndms, long long nsamps
     const double sd = (sr <= 1e-24 * (syy > 1.0 ? syy : 1.0)) ? 0.0 : sqrt(sr / dn);
     const double inv = sd > 0.0 ? 1.0 / sd : 0.0;
     // pass 2 (L2): subtract the line, normalise
-    for (long long i = threadIdx.x; i < n4; i += kThreads) {
-        float4 q = reinterpret_cast<const float4 *>(x)[i];
-        const double t = (double)(4 * i) - tbar;
-        q.x = (float)(((double)q.x - (mean + slope * t)) * inv);
-        q.y = (float)(((double)q.y - (mean + slope * (t + 1.0))) * inv);
-        q.z = (float)(((double)q.z - (mean + slope * (t + 2.0))) * inv);
-        q.w = (float)(((double)q.w - (mean + slope * (t + 3.0))) * inv);
-        reinterpret_cast<float4 *>(x)[i] = q;
+    for (long long base = 0; base < n4; base += (long long)U * kThreads) {
+        float4 qq[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kThreads + threadIdx.x;
+            qq[u] = i < n4 ? reinterpret_cast<const float4 *>(x)[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = base + (long long)u * kThreads + threadIdx.x;
+            if (i >= n4) continue;
+            float4 q = qq[u];
+            const double t = (double)(4 * i) - tbar;
+            q.x = (float)(((double)q.x - (mean + slope * t)) * inv);
+            q.y = (float)(((double)q.y - (mean + slope * (t + 1.0))) * inv);
+            q.z = (float)(((double)q.z - (mean + slope * (t + 2.0))) * inv);
+            q.w = (float)(((double)q.w - (mean + slope * (t + 3.0))) * inv);
+            reinterpret_cast<float4 *>(x)[i] = q;
+        }
     }
     for (long long t = n4 * 4 + threadIdx.x; t < n; t += kThreads)
         x[t] = (float)(((double)x[t] - (mean + slope * ((double)t - tbar))) * inv);

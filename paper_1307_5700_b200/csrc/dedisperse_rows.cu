@@ -248,7 +248,7 @@ struct RowsArgs {
     const void *y;                    // [nslots][nyrows][ystride] pre-summed rows
     void *out;
     const int4 *rowdesc;              // [nblk][nslab][CS]: (y row or -1, first staged sample - tile_t0, samples to copy, 0)
-    const uint32_t *ent;              // [nblk][nslab][DB*Q] byte offset of the (DM, group) window inside a stage (uint16: | odd)
+    const uint32_t *ent;              // [nblk][nslab][warp][Q][D] byte offset of the (DM, group) window inside a stage (uint16: | odd)
     const int32_t *sigma;             // [DB] output time shear per DM of a block
     int beam0, nslots, nyrows, ndms;
     int nblk, ntile_t, nslab, Q, ngroups, CS, pitch, stages, slabs_per_part;
@@ -358,8 +358,13 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
 #pragma unroll 1
                 for (int q = 0; q < nq; ++q) {
                     uint32_t e[D];
+                    if constexpr (D == 4) {                                             // four consecutive words: one 128-bit broadcast load
+                        const uint4 ev = *reinterpret_cast<const uint4 *>(ents + q * 4);
+                        e[0] = ev.x; e[1] = ev.y; e[2] = ev.z; e[3] = ev.w;
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < D; ++j) e[j] = ents[j * Q + q];
+                        for (int j = 0; j < D; ++j) e[j] = ents[q * D + j];
+                    }
 #pragma unroll
                     for (int j = 0; j < D; ++j) {
                         const Acc *w = reinterpret_cast<const Acc *>(sbase + e[j]) + lane;
@@ -404,8 +409,13 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
 #pragma unroll 1
                     for (int q = 0; q < nq; ++q) {
                         uint32_t e[D];
+                        if constexpr (D == 4) {
+                            const uint4 ev = *reinterpret_cast<const uint4 *>(ents + q * 4);
+                            e[0] = ev.x; e[1] = ev.y; e[2] = ev.z; e[3] = ev.w;
+                        } else {
 #pragma unroll
-                        for (int j = 0; j < D; ++j) e[j] = ents[j * Q + q];
+                            for (int j = 0; j < D; ++j) e[j] = ents[q * D + j];
+                        }               // D consecutive words: one broadcast load
 #pragma unroll
                         for (int j = 0; j < D; ++j) {
                             const uint32_t *w = reinterpret_cast<const uint32_t *>(sbase + (e[j] & ~3u)) + lane;
@@ -900,7 +910,7 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, int part_chans, cons
                     uint32_t e;
                     if (f32) e = (uint32_t)(((long long)(r + k) * pitch + o) * 4);
                     else e = (uint32_t)(((long long)(r + k) * pitch + (o & ~1LL)) * 2) | (uint32_t)(o & 1);
-                    h.ent[(((size_t)blk * nslab + slab) * DB + dl) * Q + q] = e;
+                    h.ent[((size_t)blk * nslab + slab) * DB * Q + ((size_t)(dl / g.D) * Q + q) * g.D + dl % g.D] = e;   // [warp][group][DM of the warp]
                 }
                 r += (int)u.size();
             }

@@ -295,11 +295,12 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
     __syncthreads();
 
     if (warp == NW) {
-        // ===== producer: lane r copies row r of every slab, lane 0 also the slab's slice of the entry table =====
+        // ===== producer: lane r copies rows r and r + 32 of every slab, lane 0 also the slab's slice of the entry table =====
         int st = 0;
         uint32_t ph = 1;             // parity of the empty-barrier phase to wait for (first lap: no wait)
         bool first_lap = true;
         const uint32_t smem0 = smem_u32(smem);
+        const int4 none = make_int4(-1, 0, 0, 0);
         for (long long tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
             const int blk = (int)(tile % a.nblk);
             const long long rest = tile / a.nblk;
@@ -308,23 +309,32 @@ __global__ void __launch_bounds__((Tr::NW + 1) * 32, 1) dedisperse_rows_kernel(c
             const Y *ybeam = reinterpret_cast<const Y *>(a.y) + (size_t)((a.beam0 + bb) % a.nslots) * a.nyrows * (size_t)a.ystride;
             const int4 *rd = a.rowdesc + (size_t)blk * a.nslab * a.CS;
             const uint32_t *et = a.ent + (size_t)blk * a.nslab * (DB * a.Q);
-            int4 desc = lane < a.CS ? rd[lane] : make_int4(-1, 0, 0, 0);
+            int4 desc0 = lane < a.CS ? rd[lane] : none, desc1 = lane + 32 < a.CS ? rd[lane + 32] : none;
             for (int slab = 0; slab < a.nslab; ++slab) {
-                const int4 cur = desc;
-                if (slab + 1 < a.nslab && lane < a.CS) desc = rd[(size_t)(slab + 1) * a.CS + lane];     // next slab's rows, before the wait
+                const int4 cur[2] = {desc0, desc1};
+                if (slab + 1 < a.nslab) {                                  // next slab's rows, before the wait
+                    if (lane < a.CS) desc0 = rd[(size_t)(slab + 1) * a.CS + lane];
+                    if (lane + 32 < a.CS) desc1 = rd[(size_t)(slab + 1) * a.CS + lane + 32];
+                }
                 if (!first_lap) mbar_wait_sleep(&empty[st], ph);
                 const uint32_t sbase = smem0 + st * stage_bytes;
-                uint32_t bytes = 0;
-                long long lo = 0, g0 = 0;
-                if (cur.x >= 0) {
-                    g0 = tile_t0 + cur.y;
-                    lo = g0 < 0 ? 0 : g0;
-                    long long hi = g0 + cur.z;
-                    if (hi > a.ystride) hi = a.ystride;
-                    if (hi > lo) bytes = (uint32_t)((hi - lo) * sizeof(Y));
-                }
-                mbar_arrive_expect_tx(&full[st], bytes + (lane == 0 ? ent_bytes : 0u));
-                if (bytes) bulk_g2s(sbase + lane * row_bytes + (uint32_t)((lo - g0) * sizeof(Y)), ybeam + (size_t)cur.x * a.ystride + lo, bytes, &full[st]);
+                uint32_t bytes[2] = {0, 0};
+                long long lo[2] = {0, 0}, g0[2] = {0, 0};
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+                    if (cur[k].x >= 0) {
+                        g0[k] = tile_t0 + cur[k].y;
+                        lo[k] = g0[k] < 0 ? 0 : g0[k];
+                        long long hi = g0[k] + cur[k].z;
+                        if (hi > a.ystride) hi = a.ystride;
+                        if (hi > lo[k]) bytes[k] = (uint32_t)((hi - lo[k]) * sizeof(Y));
+                    }
+                mbar_arrive_expect_tx(&full[st], bytes[0] + bytes[1] + (lane == 0 ? ent_bytes : 0u));
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+                    if (bytes[k])
+                        bulk_g2s(sbase + (lane + 32 * k) * row_bytes + (uint32_t)((lo[k] - g0[k]) * sizeof(Y)),
+                                 ybeam + (size_t)cur[k].x * a.ystride + lo[k], bytes[k], &full[st]);
                 if (lane == 0) bulk_g2s(sbase + a.CS * row_bytes, et + (size_t)slab * (DB * a.Q), ent_bytes, &full[st]);
                 if (++st == stages) { st = 0; ph ^= 1; first_lap = false; }
             }
@@ -868,7 +878,7 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, int part_chans, cons
             for (const Use &x : u) need_max = std::max(need_max, x.emax - floor_to(x.emin, al) + span);
         }
     const int pitch = (int)ceil_to(need_max, al);
-    // groups per slab: as many as keep a slab within 32 rows (one per producer lane) and three stages in shared memory
+    // groups per slab: as many as keep a slab within 64 rows (two per producer lane) and three stages in shared memory
     const int part_groups_max = f32 ? ng : std::max(1, part_chans / G);
     int Q = 0, CS = 0;
     for (int q : {4, 3, 2, 1}) {
@@ -882,7 +892,7 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, int part_chans, cons
                 cs = std::max(cs, n);
             }
         const size_t stage = (((size_t)cs * pitch * esize + (size_t)DB * q * 4) + 127) & ~(size_t)127;
-        if (cs <= 32 && 3 * stage + 256 <= kSmemBudget) { Q = q; CS = cs; break; }
+        if (cs <= 64 && 2 * stage + 256 <= kSmemBudget) { Q = q; CS = cs; break; }
     }
     if (!Q) return false;
     const int nslab = (ng + Q - 1) / Q;
@@ -1090,8 +1100,15 @@ static void free_rows_tables(RowsTables *rt)
 }
 
 // Modelled cost of a group size in units of one shared-memory operand word per output sample: nchans/G words in the
-// main kernel, plus the y rows, each written to and read back from HBM (about 14 word-times per row and sample).
-static double group_cost(const mdsm_plan *p, const GroupRows &gr) { return (double)p->ndms * gr.ngroups + 14.0 * gr.nyrows; }
+// main kernel, plus the y rows, each written to and read back from HBM.  Measured on B200 (cfg 3 and cfg 5, G = 4..8): a
+// row and sample costs about 7 word-times at the HBM copy rate; 11 also covers the slabs getting shorter (more rows per
+// group) as G grows, and reproduces the measured optimum (G = 5 at 1024 channels x 640 DMs, 6-7 at 4096 x 2048).
+// The packed 16-bit kernel (uint8 / 4-bit input) is bound by issue slots rather than by operand words and gains less
+// from wider groups: measured optimum G = 4 on cfg 4 (9.75 ms; G = 5: 10.8, G = 6: 12.3), hence the larger weight.
+static double group_cost(const mdsm_plan *p, const GroupRows &gr, bool packed16)
+{
+    return (double)p->ndms * gr.ngroups + (packed16 ? 16.0 : 11.0) * gr.nyrows;
+}
 
 static int build_dtype(mdsm_plan *p, int kind /* 0: 32-bit rows, 1: uint8 -> 16-bit rows, 2: 4-bit -> 16-bit rows */, const std::vector<GroupRows> &cands)
 {
@@ -1103,7 +1120,7 @@ static int build_dtype(mdsm_plan *p, int kind /* 0: 32-bit rows, 1: uint8 -> 16-
     // candidates in the order of their modelled cost; the first whose tables fit the kernel's limits is taken
     std::vector<const GroupRows *> order;
     for (const GroupRows &gr : cands) order.push_back(&gr);
-    std::sort(order.begin(), order.end(), [&](const GroupRows *x, const GroupRows *y) { return group_cost(p, *x) < group_cost(p, *y); });
+    std::sort(order.begin(), order.end(), [&](const GroupRows *x, const GroupRows *y) { return group_cost(p, *x, !f32) < group_cost(p, *y, !f32); });
     for (const GroupRows *gr : order) {
         RowsHost h;
         if (!build_rows_tables(p, f32, kind == 2 ? kPartChansU4 : kPartChansU8, *gr, geom, rt, h)) continue;

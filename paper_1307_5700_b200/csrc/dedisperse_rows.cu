@@ -95,6 +95,7 @@ struct PreArgs {
     const int32_t *group_row0;        // [ngroups + 1] first y row of a group
     const int16_t *ydelta;            // [nyrows][kGMax] delay of channel c0 + i relative to channel c0
     int beam0, nslots, nchans, G, nyrows, dmax;
+    int delta_off;                    // byte offset of the group's pattern table inside the dynamic shared memory
     long long nsamps, ystride;
 };
 
@@ -118,19 +119,25 @@ __global__ void __launch_bounds__(kPreThreads) group_presum_w32_kernel(const Pre
         const TIn *row = in + (size_t)(have ? c0 + i : 0) * a.nsamps;
         for (int s = threadIdx.x; s < pitch; s += kPreThreads) sm[i * pitch + s] = (have && t0 + s < a.nsamps) ? (TOut)row[t0 + s] : (TOut)0;
     }
-    __syncthreads();
+    // the group's patterns go to shared memory too: the loop below must not wait on L2 for its next deltas
     const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    int16_t *sdelta = reinterpret_cast<int16_t *>(smem_raw + a.delta_off);
+    for (int k = threadIdx.x; k < (row1 - row0) * kGMax; k += kPreThreads) sdelta[k] = a.ydelta[(size_t)row0 * kGMax + k];
+    __syncthreads();
     TOut *ybeam = reinterpret_cast<TOut *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
+    TOut x0[kPreChunkF32 / kPreThreads];                         // delta_0 = 0 for every pattern: the first channel stays in registers
+#pragma unroll
+    for (int k = 0; k < kPreChunkF32 / kPreThreads; ++k) x0[k] = sm[threadIdx.x + k * kPreThreads];
     for (int r = row0; r < row1; ++r) {
         int dl[G];
 #pragma unroll
-        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        for (int i = 0; i < G; ++i) dl[i] = sdelta[(r - row0) * kGMax + i];
         TOut *yrow = ybeam + (size_t)r * a.ystride + t0;
         TOut v[kPreChunkF32 / kPreThreads];
 #pragma unroll
         for (int k = 0; k < kPreChunkF32 / kPreThreads; ++k) {
             const int s = threadIdx.x + k * kPreThreads;
-            TOut acc = sm[s];                                    // delta_0 = 0
+            TOut acc = x0[k];
 #pragma unroll
             for (int i = 1; i < G; ++i) acc += sm[i * pitch + s + dl[i]];
             v[k] = acc;
@@ -174,13 +181,15 @@ __global__ void __launch_bounds__(kPreThreads) group_presum_u8_kernel(const PreA
             for (int s = threadIdx.x; s < pitch; s += kPreThreads) smem_raw[i * pitch + s] = (have && t0 + s < a.nsamps) ? row[t0 + s] : (uint8_t)0;
         }
     }
-    __syncthreads();
     const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    int16_t *sdelta = reinterpret_cast<int16_t *>(smem_raw + a.delta_off);
+    for (int k = threadIdx.x; k < (row1 - row0) * kGMax; k += kPreThreads) sdelta[k] = a.ydelta[(size_t)row0 * kGMax + k];
+    __syncthreads();
     uint16_t *ybeam = reinterpret_cast<uint16_t *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
     for (int r = row0; r < row1; ++r) {
         int dl[G];
 #pragma unroll
-        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        for (int i = 0; i < G; ++i) dl[i] = sdelta[(r - row0) * kGMax + i];
         uint16_t *yrow = ybeam + (size_t)r * a.ystride + t0;
 #pragma unroll
         for (int k = 0; k < kPreChunkU8 / (4 * kPreThreads); ++k) {
@@ -218,13 +227,15 @@ __global__ void __launch_bounds__(kPreThreads) group_presum_u4_kernel(const PreA
         const uint8_t *row = in + (size_t)(have ? c0 + i : 0) * row_bytes;
         for (int s = threadIdx.x; s < pitch; s += kPreThreads) smem_raw[i * pitch + s] = (have && t0 / 2 + s < row_bytes) ? row[t0 / 2 + s] : (uint8_t)0;
     }
-    __syncthreads();
     const int row0 = a.group_row0[g], row1 = a.group_row0[g + 1];
+    int16_t *sdelta = reinterpret_cast<int16_t *>(smem_raw + a.delta_off);
+    for (int k = threadIdx.x; k < (row1 - row0) * kGMax; k += kPreThreads) sdelta[k] = a.ydelta[(size_t)row0 * kGMax + k];
+    __syncthreads();
     uint16_t *ybeam = reinterpret_cast<uint16_t *>(a.y) + (size_t)(b % a.nslots) * a.nyrows * (size_t)a.ystride;
     for (int r = row0; r < row1; ++r) {
         int dl[G];
 #pragma unroll
-        for (int i = 0; i < G; ++i) dl[i] = a.ydelta[(size_t)r * kGMax + i];
+        for (int i = 0; i < G; ++i) dl[i] = sdelta[(r - row0) * kGMax + i];
         uint16_t *yrow = ybeam + (size_t)r * a.ystride + t0;
 #pragma unroll
         for (int k = 0; k < kPreChunkU8 / (4 * kPreThreads); ++k) {
@@ -788,7 +799,7 @@ template <typename V> static bool upload(V **dptr, const std::vector<V> &h)
 
 // y rows of a group size: every pattern of relative delays a group takes over the DM grid
 struct GroupRows {
-    int G = 0, ngroups = 0, nyrows = 0, dmax = 0;
+    int G = 0, ngroups = 0, nyrows = 0, dmax = 0, maxpat = 0;  // maxpat: most rows of one group
     std::vector<int32_t> yrow_of;          // [ndms][ngroups]
     std::vector<int32_t> group_row0;       // [ngroups + 1]
     std::vector<int16_t> ydelta;           // [nyrows][kGMax]
@@ -834,6 +845,8 @@ static bool enumerate_group_rows(const mdsm_plan *p, int G, GroupRows &gr)
     }
     gr.group_row0[gr.ngroups] = nrows;
     gr.nyrows = nrows;
+    gr.maxpat = 0;
+    for (int g = 0; g < gr.ngroups; ++g) gr.maxpat = std::max(gr.maxpat, gr.group_row0[g + 1] - gr.group_row0[g]);
     return true;
 }
 
@@ -928,6 +941,7 @@ static bool build_rows_tables(const mdsm_plan *p, bool f32, int part_chans, cons
     rt.G = G; rt.D = g.D; rt.T = g.T; rt.NW = g.NW; rt.DB = DB; rt.span = span; rt.stride = stride;
     rt.Q = Q; rt.CS = CS; rt.pitch = pitch; rt.nslab = nslab; rt.nblk = nblk; rt.ngroups = ng; rt.nyrows = gr.nyrows;
     rt.dmax = gr.dmax;
+    rt.maxpat = gr.maxpat;
     rt.slabs_per_part = f32 ? nslab : part_groups_max / Q;
     rt.ystride = ceil_to(p->nsamps, al);
     rt.sigma_max = *std::max_element(h.sigma.begin(), h.sigma.end());
@@ -1222,26 +1236,28 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
     const int chunk = w32 ? kPreChunkF32 : kPreChunkU8;
     const size_t pre_smem = w32 ? (size_t)rt.G * (chunk + rt.dmax) * 4
                                 : (dtype == MDSM_U8 ? (size_t)rt.G * (chunk + ((rt.dmax + 3) & ~3) + 4) : (size_t)rt.G * ((((chunk + rt.dmax) / 2 + 3) & ~3) + 8));
-    MDSM_REQUIRE(pre_smem <= 200 * 1024, "pre-pass: group delay range too large");
+    const size_t delta_off = (pre_smem + 15) & ~(size_t)15;
+    const size_t pre_smem_all = delta_off + (size_t)rt.maxpat * kGMax * sizeof(int16_t);
+    MDSM_REQUIRE(pre_smem_all <= 200 * 1024, "pre-pass: group delay range or pattern count too large");
     // beams go through the scratch `nslots` at a time (slot = beam % nslots), in stream order
     for (int bs = beam0; bs < beam0 + nb; bs += nslots) {
         const int n = std::min(nslots, beam0 + nb - bs);
         PreArgs pa;
         pa.in = d_in; pa.y = scratch; pa.group_row0 = rt.d_group_row0; pa.ydelta = rt.d_ydelta;
         pa.beam0 = bs; pa.nslots = nslots; pa.nchans = p->nchans; pa.G = rt.G; pa.nyrows = rt.nyrows; pa.dmax = rt.dmax;
-        pa.nsamps = p->nsamps; pa.ystride = rt.ystride;
+        pa.nsamps = p->nsamps; pa.ystride = rt.ystride; pa.delta_off = (int)delta_off;
         dim3 grid((unsigned)((rt.ystride + chunk - 1) / chunk), rt.ngroups, n);
         MDSM_REQUIRE(rt.ngroups <= 65535 && n <= 65535, "pre-pass: grid too large");
         cudaError_t pe;
         switch (rt.G) {
-            case 1: pe = launch_presum<1>(dtype, pa, grid, pre_smem, st); break;
-            case 2: pe = launch_presum<2>(dtype, pa, grid, pre_smem, st); break;
-            case 3: pe = launch_presum<3>(dtype, pa, grid, pre_smem, st); break;
-            case 4: pe = launch_presum<4>(dtype, pa, grid, pre_smem, st); break;
-            case 5: pe = launch_presum<5>(dtype, pa, grid, pre_smem, st); break;
-            case 6: pe = launch_presum<6>(dtype, pa, grid, pre_smem, st); break;
-            case 7: pe = launch_presum<7>(dtype, pa, grid, pre_smem, st); break;
-            default: pe = launch_presum<8>(dtype, pa, grid, pre_smem, st); break;
+            case 1: pe = launch_presum<1>(dtype, pa, grid, pre_smem_all, st); break;
+            case 2: pe = launch_presum<2>(dtype, pa, grid, pre_smem_all, st); break;
+            case 3: pe = launch_presum<3>(dtype, pa, grid, pre_smem_all, st); break;
+            case 4: pe = launch_presum<4>(dtype, pa, grid, pre_smem_all, st); break;
+            case 5: pe = launch_presum<5>(dtype, pa, grid, pre_smem_all, st); break;
+            case 6: pe = launch_presum<6>(dtype, pa, grid, pre_smem_all, st); break;
+            case 7: pe = launch_presum<7>(dtype, pa, grid, pre_smem_all, st); break;
+            default: pe = launch_presum<8>(dtype, pa, grid, pre_smem_all, st); break;
         }
         MDSM_CUDA_TRY(pe);
         MDSM_CUDA_TRY(cudaGetLastError());

@@ -34,7 +34,7 @@ struct RowsTables {
     int D = 0, T = 0, NW = 0, DB = 0;             // DMs per warp, words per thread and DM, consumer warps, DMs per block
     int span = 0, stride = 0;                     // samples a tile's accumulators cover per DM / outputs it owns (its time step)
     int Q = 0, CS = 0, pitch = 0;                 // groups per slab, row slots per stage, elements per row slot
-    int nslab = 0, nblk = 0, ngroups = 0, nyrows = 0, dmax = 0, slabs_per_part = 0;
+    int nslab = 0, nblk = 0, ngroups = 0, nyrows = 0, dmax = 0, maxpat = 0, slabs_per_part = 0;
     long long ystride = 0;                        // elements per y row (nsamps rounded up to 16 bytes)
     int sigma_max = 0, stages = 0;
     size_t smem_bytes = 0;

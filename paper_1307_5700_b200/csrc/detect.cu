@@ -264,7 +264,8 @@ detect_fused_kernel(const T *__restrict__ out, int beam0, int ndms, long long ns
     }
     const long long nchunks = (n4 + 31) / 32;
     for (long long c = warp; c < nchunks; c += kFusedThreads / 32)
-        if (all || cmax[c] > cb) threshold_emit4<T>(x, n, (c * 32 + lane) * 4, b, d, mean, rms, thr, cut, events, max_events, count);
+        if (all || cmax[c] > cb)                                  // the vector part only (n4 * 4 samples): the rest follows below
+            threshold_emit4<T>(x, n4 * 4, (c * 32 + lane) * 4, b, d, mean, rms, thr, cut, events, max_events, count);
     // what the vector loop did not cover (an unaligned row: everything; else the last n % 4 samples)
     for (long long t0 = n4 * 4 + (long long)threadIdx.x * 4; t0 - (long long)lane * 4 < n; t0 += (long long)kFusedThreads * 4)
         threshold_emit4<T>(x, n, t0, b, d, mean, rms, thr, cut, events, max_events, count);

@@ -303,3 +303,30 @@ def test_tmem_operand_variant_matches_the_oracle(name):
         out = p.dedisperse(torch.from_numpy(x).cuda(), kernel=3)
         assert_f32_parity(out_to_numpy(out, p.nsamps_out), ref, ab, name)
         assert np.all(out[:, :, p.nsamps_out:].cpu().numpy() == -7)
+
+
+@pytest.mark.parametrize("ns", [6000, 6003, 70001])
+def test_detect_one_launch_and_two_launch_forms_agree_with_the_oracle(ns):
+    """mdsm_detect is one launch (chunk maxima + revisits) by default; option detect_two_pass keeps the two-launch form.
+    Both must give the oracle's events bit for bit on uint32 series, for aligned and unaligned rows, negative thresholds
+    (every sample is a candidate) and series longer than one pass of the CTA."""
+    torch = _torch()
+    g = np.random.default_rng(ns)
+    nb, nd = 2, 5
+    args = (nb, 8, 418.0, -2.5, 51.2e-6, ns, 0.0, 0.15, nd)
+    with Plan(args) as p:
+        n = p.nsamps_out
+        s = np.rint(g.normal(size=(nb, nd, ns)) * 40 + 4000).astype(np.uint32)
+        s[1, 3, 17] += 900
+        s[0, 0, n - 1] += 700
+        s[0, 2, n - 2:n] += 500
+        s[1, 4, :] = 77
+        d = torch.from_numpy(s.view(np.int32)).cuda()
+        for thr in (3.0, -0.5):
+            ev_o, cnt_o, _ = oracle.detect(s, n, thr)
+            for two_pass in (0, 1):
+                p.set_option("detect_two_pass", two_pass)
+                l0 = p.m.mdsm_plan_launch_count(p.h)
+                ev_g, cnt_g = p.detect(d, thr, max_events=1 << 21)
+                assert p.m.mdsm_plan_launch_count(p.h) - l0 == (2 if two_pass else 1)
+                assert cnt_g == cnt_o and np.array_equal(ev_g, ev_o)

@@ -81,3 +81,32 @@ def test_bandpass_stage_argument_errors():
             p.m.mdsm_bandpass_clip(p.h, d, 0, 1, 64, 16, 5.0, 5.0, 5.0, False)      # order >= nchans
         with pytest.raises(p.m.MdsmError):
             p.m.mdsm_bandpass_clip(p.h, d, 0, 2, 64, 2, 5.0, 5.0, 5.0, False)       # beam range
+
+
+@pytest.mark.parametrize("shape", [(1, 2, 256, 256, 0), (1, 3, 1001, 7, 1), (2, 5, 96, 1, 2), (1, 64, 2048, 2048, 5)])
+def test_bandpass_stage_degenerate_shapes(shape):
+    """Few channels (order < nchans), one chunk per channel, window 1, rows that are not 16-byte aligned."""
+    import torch
+    nb, nc, ns, window, order = shape
+    g = np.random.default_rng(nc * 1000 + ns)
+    x = (g.exponential(size=(nb, nc, ns)) * (5.0 + np.arange(nc))[None, :, None]).astype(np.float32)
+    x[:, :, ns // 3] += 40.0
+    xo = x.copy()
+    ref = oracle.bandpass_clip(xo, window, order, 5.0, 30.0, 1.0, True)
+    args = (nb, nc, 418.0, -20.0 / nc, 51.2e-6, ns, 0.0, 0.01, 2)
+    with Plan(args) as p:
+        d = torch.from_numpy(x).cuda()
+        cm = torch.zeros((nb, nc, ns // window), dtype=torch.uint8, device="cuda")
+        sm = torch.zeros((nb, ns), dtype=torch.uint8, device="cuda")
+        fit = torch.zeros((nb, nc, 2), dtype=torch.float64, device="cuda")
+        st = torch.zeros((nb, 4), dtype=torch.float64, device="cuda")
+        p.m.mdsm_bandpass_clip(p.h, d, 0, nb, window, order, 5.0, 30.0, 1.0, True, cm, sm, fit, st)
+        torch.cuda.synchronize()
+        f = fit.cpu().numpy()
+        assert np.allclose(f[:, :, 0], ref["fit"], rtol=1e-8, atol=1e-10)
+        assert np.array_equal(st.cpu().numpy()[:, 3].astype(int), ref["nmasked"])
+        same_c = np.array_equal(cm.cpu().numpy(), ref["chan_mask"])
+        same_s = np.array_equal(sm.cpu().numpy(), ref["spec_mask"])
+        assert (cm.cpu().numpy() != ref["chan_mask"]).mean() < 1e-3 and (sm.cpu().numpy() != ref["spec_mask"]).mean() < 1e-3
+        if same_c and same_s:
+            assert np.allclose(d.cpu().numpy(), xo, rtol=0, atol=np.abs(ref["fit"]).max() * 2.0 ** -22)

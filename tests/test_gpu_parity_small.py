@@ -305,7 +305,7 @@ def test_tmem_operand_variant_matches_the_oracle(name):
         assert np.all(out[:, :, p.nsamps_out:].cpu().numpy() == -7)
 
 
-@pytest.mark.parametrize("ns", [6000, 6003, 70001])
+@pytest.mark.parametrize("ns", [40, 131, 6000, 6003, 70001])
 def test_detect_one_launch_and_two_launch_forms_agree_with_the_oracle(ns):
     """mdsm_detect is one launch (chunk maxima + revisits) by default; option detect_two_pass keeps the two-launch form.
     Both must give the oracle's events bit for bit on uint32 series, for aligned and unaligned rows, negative thresholds
@@ -317,7 +317,7 @@ def test_detect_one_launch_and_two_launch_forms_agree_with_the_oracle(ns):
     with Plan(args) as p:
         n = p.nsamps_out
         s = np.rint(g.normal(size=(nb, nd, ns)) * 40 + 4000).astype(np.uint32)
-        s[1, 3, 17] += 900
+        s[1, 3, min(17, n - 1)] += 900
         s[0, 0, n - 1] += 700
         s[0, 2, n - 2:n] += 500
         s[1, 4, :] = 77

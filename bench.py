@@ -352,7 +352,31 @@ def bench_postprocess(m, torch, cfg, args, plan, work, pristine, out, nso, strea
         tp.append(pe[0].elapsed_time(pe[1]))
     post["power_ms"] = statistics.mean(tp[1:])
     post["power_hbm_frac"] = 8.0 * nel / (post["power_ms"] * 1e-3) / hp
-    del volt
+    # the 4-bit quantiser of the complex voltages (NEXT-4): 2 x 4 B read (max pass + coding pass) + 1 B written per sample
+    packed = torch.empty((nel,), dtype=torch.uint8, device="cuda")
+    xthr = torch.zeros(9, dtype=torch.int32, device="cuda")
+    tc = []
+    for _ in range(5):
+        out.zero_()
+        pe[0].record(stream)
+        m.mdsm_mulaw_c4(volt, packed, nel, 255.0, xthr, stream)
+        pe[1].record(stream)
+        torch.cuda.synchronize()
+        tc.append(pe[0].elapsed_time(pe[1]))
+    post["mulaw_c4_ms"] = statistics.mean(tc[1:])
+    post["mulaw_c4_hbm_frac"] = 9.0 * nel / (post["mulaw_c4_ms"] * 1e-3) / hp
+    del volt, packed
+    # the paper's bandpass-fit RFI stage (NEXT-2) on the buffer of the workload: floor = one read + one write of the input
+    tb = []
+    for _ in range(4):
+        work.copy_(pristine)
+        pe[0].record(stream)
+        m.mdsm_bandpass_clip(plan, work, 0, cfg.nbeams, cfg.window, 4, 5.0, 50.0, 5.0, True, None, None, None, None, stream)
+        pe[1].record(stream)
+        torch.cuda.synchronize()
+        tb.append(pe[0].elapsed_time(pe[1]))
+    post["bandpass_clip_ms"] = statistics.mean(tb[1:])
+    post["bandpass_clip_hbm_frac"] = 8.0 * nel / (post["bandpass_clip_ms"] * 1e-3) / hp
     # mu-law quantiser (Eq. 5, NEXT-4) on the fp32 input buffer (power is non-negative: use |x|)
     src = work.abs_()
     codes = torch.empty((nel,), dtype=torch.uint8, device="cuda")

@@ -499,27 +499,41 @@ bp_fit_kernel(const double *__restrict__ bp_all, int beam0, int nchans, int npad
     }
 }
 
-// H6 + H7.  Thread = one time sample x kChPer channels (coalesced along t).
+// H6 + H7.  Thread = V consecutive time samples (V = 4: one 128-bit access, aligned rows; else 1) x kBpChPer channels.
 constexpr int kBpChPer = 16;
+template <int V>
 __global__ void __launch_bounds__(kThreads)
 bp_spec_apply_kernel(float *__restrict__ in, int beam0, int nchans, long long nsamps, const double *__restrict__ spec_sum,
                      const double *__restrict__ spec_stats, const double *__restrict__ chan_stats, int subtract,
                      uint8_t *__restrict__ spec_mask)
 {
     const int b = beam0 + blockIdx.z;
-    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const long long t = ((long long)blockIdx.x * kThreads + threadIdx.x) * V;
     if (t >= nsamps) return;
-    const bool flag = __ddiv_rn(spec_sum[(size_t)b * nsamps + t], (double)nchans) > spec_stats[4 * b];
-    if (blockIdx.y == 0 && spec_mask) spec_mask[(size_t)b * nsamps + t] = flag ? 1 : 0;
-    if (!flag && !subtract) return;
+    const double thr = spec_stats[4 * b];
+    bool flag[V], any = false;
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        flag[k] = __ddiv_rn(spec_sum[(size_t)b * nsamps + t + k], (double)nchans) > thr;
+        any |= flag[k];
+        if (blockIdx.y == 0 && spec_mask) spec_mask[(size_t)b * nsamps + t + k] = flag[k] ? 1 : 0;
+    }
+    if (!any && !subtract) return;
     const int c0 = blockIdx.y * kBpChPer, c1 = min(nchans, c0 + kBpChPer);
     float *col = in + ((size_t)b * nchans + c0) * (size_t)nsamps + t;
     const double *st = chan_stats + ((size_t)b * nchans + c0) * 4;
     for (int c = c0; c < c1; ++c, col += nsamps, st += 4) {
         const float f = (float)st[3];
-        float v = flag ? f : *col;
-        if (subtract) v = v - f;
-        *col = v;
+        if (V == 4) {
+            float4 v = *reinterpret_cast<float4 *>(col);
+            v.x = flag[0] ? f : v.x; v.y = flag[1] ? f : v.y; v.z = flag[2] ? f : v.z; v.w = flag[3] ? f : v.w;
+            if (subtract) { v.x = v.x - f; v.y = v.y - f; v.z = v.z - f; v.w = v.w - f; }
+            *reinterpret_cast<float4 *>(col) = v;
+        } else {
+            float v = flag[0] ? f : *col;
+            if (subtract) v = v - f;
+            *col = v;
+        }
     }
 }
 
@@ -620,10 +634,13 @@ int mdsm_launch_bandpass_clip(mdsm_plan *p, float *in, int beam0, int nb, int wi
         clip_spec_sum_kernel<float, false><<<grid2, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum);
     }
     MDSM_CUDA_TRY(cudaGetLastError());
-    dim3 grid4((unsigned)((nsamps + kThreads - 1) / kThreads), (unsigned)((p->nchans + kBpChPer - 1) / kBpChPer), nb);
+    const int V = aligned ? 4 : 1;
+    dim3 grid4((unsigned)((nsamps + (long long)kThreads * V - 1) / ((long long)kThreads * V)), (unsigned)((p->nchans + kBpChPer - 1) / kBpChPer), nb);
     MDSM_REQUIRE(grid4.y <= 65535 && nb <= 65535, "bandpass stage: grid too large");
-    bp_spec_apply_kernel<<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats, p->d_chan_stats, subtract,
-                                                    spec_mask);
+    if (aligned)
+        bp_spec_apply_kernel<4><<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats, p->d_chan_stats, subtract, spec_mask);
+    else
+        bp_spec_apply_kernel<1><<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats, p->d_chan_stats, subtract, spec_mask);
     MDSM_CUDA_TRY(cudaGetLastError());
     p->launches += 5;
     return MDSM_OK;

@@ -38,16 +38,14 @@ template <> struct Elem<uint8_t> {
     using Acc = unsigned long long;
     __device__ static void sums(const Vec &v, Acc &s, Acc &q)
     {
+        // four bytes per instruction: dp4a with ones gives the sum, with the word itself the sum of squares (exact in 32 bits)
         unsigned ss = 0, qq = 0;
         const unsigned w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                unsigned e = (w[i] >> (8 * k)) & 0xffu;
-                ss += e;
-                qq += e * e;
-            }
+        for (int i = 0; i < 4; ++i) {
+            ss = __dp4a(w[i], 0x01010101u, ss);
+            qq = __dp4a(w[i], w[i], qq);
+        }
         s = ss;
         q = qq;
     }
@@ -298,21 +296,24 @@ clip_spec_stats_kernel(const double *__restrict__ spec_sum, int beam0, long long
     }
 }
 
+// Thread = one time sample x kApplyChPer channels: a flagged spectrum is overwritten by nchans / kApplyChPer threads side by side.
+constexpr int kApplyChPer = 128;
 template <typename T>
 __global__ void __launch_bounds__(kThreads)
 clip_spec_apply_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps, const double *__restrict__ spec_sum,
                        const double *__restrict__ spec_stats, const double *__restrict__ chan_stats,
                        uint8_t *__restrict__ spec_mask)
 {
-    const int b = beam0 + blockIdx.y;
+    const int b = beam0 + blockIdx.z;
     const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
     if (t >= nsamps) return;
     const bool flag = spec_sum[(size_t)b * nsamps + t] > spec_stats[4 * b];
-    if (spec_mask) spec_mask[(size_t)b * nsamps + t] = flag ? 1 : 0;
+    if (blockIdx.y == 0 && spec_mask) spec_mask[(size_t)b * nsamps + t] = flag ? 1 : 0;
     if (flag) {
-        T *col = in + (size_t)b * nchans * (size_t)nsamps + t;
-        const double *st = chan_stats + (size_t)b * nchans * 4;
-        for (int c = 0; c < nchans; ++c) col[(size_t)c * nsamps] = (T)st[4 * c + 3];
+        const int c0 = blockIdx.y * kApplyChPer, c1 = min(nchans, c0 + kApplyChPer);
+        T *col = in + ((size_t)b * nchans + c0) * (size_t)nsamps + t;
+        const double *st = chan_stats + ((size_t)b * nchans + c0) * 4;
+        for (int c = c0; c < c1; ++c, col += nsamps, st += 4) *col = (T)st[3];
     }
 }
 
@@ -574,7 +575,8 @@ int launch_clip_t(mdsm_plan *p, T *in, int beam0, int nb, int window, double k_c
     MDSM_CUDA_TRY(cudaGetLastError());
     clip_spec_stats_kernel<sizeof(T) == 1><<<nb, 1024, 0, st>>>(p->d_spec_sum, beam0, nsamps, k_spec, spec_stats);
     MDSM_CUDA_TRY(cudaGetLastError());
-    dim3 grid4((unsigned)((nsamps + kThreads - 1) / kThreads), nb);
+    dim3 grid4((unsigned)((nsamps + kThreads - 1) / kThreads), (unsigned)((p->nchans + kApplyChPer - 1) / kApplyChPer), nb);
+    MDSM_REQUIRE(grid4.y <= 65535 && nb <= 65535, "clip: grid too large");
     clip_spec_apply_kernel<T><<<grid4, kThreads, 0, st>>>(in, beam0, p->nchans, nsamps, p->d_spec_sum, spec_stats,
                                                           p->d_chan_stats, spec_mask);
     MDSM_CUDA_TRY(cudaGetLastError());

@@ -29,7 +29,7 @@ template <> struct Elem<float> {
     {
         double a = v.x, b = v.y, c = v.z, d = v.w;
         s = (a + b) + (c + d);
-        q = (a * a + b * b) + (c * c + d * d);
+        q = fma(a, a, fma(b, b, fma(c, c, d * d)));
     }
 };
 template <> struct Elem<uint8_t> {
@@ -108,6 +108,31 @@ clip_channel_kernel(T *__restrict__ in, int beam0, int nchans, long long nsamps,
         const int gshift = __ffs(g) - 1;
         const long long nvec = nsamps / V;
         const typename E::Vec *vrow = reinterpret_cast<const typename E::Vec *>(row);
+        if (sizeof(T) == 4 && g >= 4) {
+            // float rows: a thread takes FOUR consecutive vectors of a chunk, so that the fp64 shuffle tree over the chunk's
+            // lanes is two levels shorter (the kernel is bound by instruction issue, not by memory)
+            const int g4 = g >> 2;
+            for (long long base = 0; base < nvec; base += 4LL * kThreads) {
+                const long long i0 = base + 4LL * tid;
+                Acc s = 0, q = 0;
+                if (i0 < nvec) {                               // nvec is a multiple of g, g of 4: all four or none
+                    typename E::Vec v[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) v[k] = vrow[i0 + k];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        Acc s1, q1;
+                        E::sums(v[k], s1, q1);
+                        s += s1;
+                        q += q1;
+                    }
+                }
+                S += s;
+                Q += q;
+                for (int m = 1; m < g4; m <<= 1) s += shfl_xor<Acc>(s, m);
+                if (i0 < nvec && (lane & (g4 - 1)) == 0) csum[i0 >> gshift] = (double)s;
+            }
+        } else
         for (long long base = 0; base < nvec; base += kThreads) {
             const long long i = base + tid;
             Acc s = 0, q = 0;

@@ -156,6 +156,45 @@ int mdsm_detect(mdsm_plan *plan, const void *d_out, int dtype, int beam0, int nb
                 double snr_thresh, mdsm_event *d_events, int64_t max_events,
                 unsigned long long *d_count, void *cuda_stream);
 
+/* mdsm_detect for callers that are not able to allocate device memory -- the same n-sigma thresholding (PAPER.md:116,
+ * normalisation PAPER.md:110), same events, but it needs NO plan and calls no cudaMalloc / cudaFree / allocating library
+ * routine, neither at set-up nor per call.
+ *
+ * Who this is for.  Every other stage call wants an mdsm_plan, and mdsm_plan_create / mdsm_plan_reserve obtain their
+ * device memory with cudaMalloc.  Some users of the detection step cannot do that:
+ *   - a plug-in inside a host application (an acquisition or correlator process, a framework with its own caching
+ *     allocator) that has already claimed the device's memory and hands the plug-in fixed input / output buffers:
+ *     a further cudaMalloc there fails, or takes memory the host has budgeted for something else;
+ *   - the soft-real-time loop of the paper itself: cudaMalloc and cudaFree synchronise the whole
+ *     device, so a thread that allocates while other beams' buffers are in flight stalls all of them and can make
+ *     the pipeline miss its buffer deadline.
+ * The per-series mean / rms pairs that detection keeps between its two kernels therefore live in a fixed array
+ * inside libmdsm.so's device image (`static __device__`, 16 bytes x MDSM_DETECT_NOALLOC_MAX_SERIES = 512 KB).  The
+ * CUDA runtime places that array on every GPU on which the library's kernels are loaded and keeps it there until the
+ * process exits; that is the price of never allocating.
+ *
+ *   d_series [nbeams][ndms][nsamps]  float (MDSM_F32) or uint32_t (MDSM_U8), device, caller-owned, any alignment; the first
+ *                                    nsamps_out (1 <= nsamps_out <= nsamps) samples of a row are thresholded, as in mdsm_detect;
+ *   d_events, max_events, d_count    exactly as in mdsm_detect (the caller zeroes *d_count; events carry beam 0 .. nbeams-1).
+ * Limit: nbeams * ndms <= MDSM_DETECT_NOALLOC_MAX_SERIES (enough for 16 beams x 2048 DM trials, the largest
+ * configuration this library is measured on); beyond that the call does nothing and returns MDSM_EINVAL with a message that
+ * names the limit -- split the series into several calls then, one after the other on ONE stream.
+ * First call: the first call on each device (with that device current) asks the runtime for the device address of the
+ * array and remembers it; later calls only launch the two kernels.  Make that first call during start-up, before any
+ * stream capture begins on the device.
+ * Shared state: all calls on a device use the same array.  It still holds the previous call's means and rms values; no
+ * element has to start at zero, because each call first writes the nbeams * ndms pairs it then reads.  For the same reason
+ * two calls whose kernels may run on the GPU at the same time (different streams, different host threads) RACE and
+ * produce wrong events: issue them on one stream, or order them with events.
+ * Asynchronous on cuda_stream like mdsm_detect; runs the statistics + thresholding kernels as two launches (the
+ * "detect_two_pass" form), so any series length is accepted.  Errors: MDSM_EINVAL (null pointers, dtype other than
+ * MDSM_F32 / MDSM_U8, sizes < 1, nsamps_out > nsamps, NaN threshold, ndms or nbeams > 65535, too many series),
+ * MDSM_ECUDA (the address query or a launch failed). */
+#define MDSM_DETECT_NOALLOC_MAX_SERIES 32768
+int mdsm_detect_noalloc(const void *d_series, int dtype, int nbeams, int ndms, int64_t nsamps, int64_t nsamps_out,
+                        double snr_thresh, mdsm_event *d_events, int64_t max_events, unsigned long long *d_count,
+                        void *cuda_stream);
+
 /* Post-processing of the dedispersed series between mdsm_dedisperse and mdsm_detect (section
  * 2.2.3: "optional post-processing").  fp32 series only, layout of d_out ([nbeams][ndms][nsamps], the
  * first nsamps_out samples of a row valid); device pointers, asynchronous on cuda_stream, no allocation.

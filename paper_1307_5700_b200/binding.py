@@ -20,10 +20,12 @@ __all__ = [
     "mdsm_plan_reserve", "mdsm_plan_kernel_info",
     "mdsm_rfi_clip", "mdsm_bandpass_clip", "mdsm_dedisperse", "mdsm_detect", "mdsm_median_filter", "mdsm_detrend", "mdsm_power_i16", "mdsm_mulaw_u8", "mdsm_pipeline_host", "mdsm_measure_add_peak",
     "mdsm_cluster_events", "mdsm_classify_clusters", "mdsm_mulaw_c4",
+    "mdsm_detect_noalloc", "MDSM_DETECT_NOALLOC_MAX_SERIES",
 ]
 
 MDSM_F32, MDSM_U8, MDSM_U16, MDSM_U4 = 0, 1, 2, 3
 MDSM_OK, MDSM_EINVAL, MDSM_ENOMEM, MDSM_ECUDA, MDSM_EOVERFLOW = 0, -1, -2, -3, 1
+MDSM_DETECT_NOALLOC_MAX_SERIES = 32768      # the #define of include/mdsm.h (a test keeps the two equal)
 EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -97,6 +99,9 @@ def _load():
                                      c_int64, POINTER(c_uint64), c_int]
     L.mdsm_measure_add_peak.restype = c_int
     L.mdsm_measure_add_peak.argtypes = [c_int, POINTER(c_double)]
+    L.mdsm_detect_noalloc.restype = c_int
+    L.mdsm_detect_noalloc.argtypes = [c_void_p, c_int, c_int, c_int, c_int64, c_int64, c_double, c_void_p, c_int64, c_void_p,
+                                      c_void_p]
     return L
 
 
@@ -220,6 +225,16 @@ def mdsm_dedisperse(plan, d_in, beam0, nb, d_out, stream=None, dtype=None) -> No
 def mdsm_detect(plan, d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, stream=None, dtype=None) -> None:
     _check(_L.mdsm_detect(plan, _ptr(d_out), _dtype_of(d_out, dtype), beam0, nb, snr_thresh, _ptr(d_events),
                           max_events, _ptr(d_count), _stream(stream)))
+
+
+def mdsm_detect_noalloc(d_series, nbeams, ndms, nsamps, nsamps_out, snr_thresh, d_events, max_events, d_count, stream=None,
+                        dtype=None) -> None:
+    """mdsm_detect without a plan and without any device allocation inside the library, for callers that cannot call
+    cudaMalloc (a plug-in in a process whose host application owns the GPU memory; a real-time loop that cannot afford
+    cudaMalloc's device-wide stall).  At most MDSM_DETECT_NOALLOC_MAX_SERIES = nbeams * ndms series per call; calls
+    share one fixed scratch array per GPU, so do not let two of them overlap on the device.  See include/mdsm.h."""
+    _check(_L.mdsm_detect_noalloc(_ptr(d_series), _dtype_of(d_series, dtype), nbeams, ndms, nsamps, nsamps_out, snr_thresh,
+                                  _ptr(d_events), max_events, _ptr(d_count), _stream(stream)))
 
 
 def mdsm_median_filter(plan, d_series, d_filtered, beam0, nb, window, stream=None) -> None:

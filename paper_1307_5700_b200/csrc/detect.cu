@@ -307,3 +307,85 @@ int mdsm_launch_detect(mdsm_plan *p, const void *d_out, int dtype, int beam0, in
         return launch_detect_t<float>(p, (const float *)d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, st);
     return launch_detect_t<uint32_t>(p, (const uint32_t *)d_out, beam0, nb, snr_thresh, d_events, max_events, d_count, st);
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// mdsm_detect_noalloc (include/mdsm.h): detection for callers that must not allocate device memory -- plug-ins that
+// live inside a host application which owns the GPU's memory, and real-time loops in which cudaMalloc's device-wide
+// synchronisation would stall the other beams.  It is the two-launch form above (series_stats_kernel, then
+// threshold_emit_kernel) with the (mean, rms) pairs the first kernel hands to the second kept in a fixed array of the
+// library's device image instead of plan-owned cudaMalloc memory.  No plan, no cudaMalloc / cudaFree.
+//
+// g_noalloc_series_stats is resident on every GPU that loads this module, until the process exits (512 KB each).
+// In HOST code the name below is only a handle for the runtime, not a device address: handing it to a kernel as a
+// pointer would fault, or quietly touch host memory on systems where the GPU can reach it.  noalloc_scratch() turns it
+// into the real device address once per device with cudaGetSymbolAddress and the launches use that address.
+#include <mutex>
+
+namespace {
+
+static __device__ __align__(256) double g_noalloc_series_stats[2 * (size_t)MDSM_DETECT_NOALLOC_MAX_SERIES];
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+double *g_noalloc_addr[kNoallocMaxDevices] = {};           // device address of the array, per device ordinal; 0 = not asked yet
+
+// Device address of the array on the CURRENT device.  The first call per device asks the runtime (which loads this
+// library's module on that device if no kernel of it ran there before); later calls read the table.
+int noalloc_scratch(double **addr)
+{
+    int dev = -1;
+    MDSM_CUDA_TRY(cudaGetDevice(&dev));
+    MDSM_REQUIRE(dev >= 0 && dev < kNoallocMaxDevices, "mdsm_detect_noalloc: device ordinal %d outside 0..%d", dev,
+                 kNoallocMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[dev]) {
+        void *a = nullptr;
+        MDSM_CUDA_TRY(cudaGetSymbolAddress(&a, g_noalloc_series_stats));
+        MDSM_REQUIRE(a != nullptr, "mdsm_detect_noalloc: the runtime returned a null address for the scratch array");
+        g_noalloc_addr[dev] = static_cast<double *>(a);
+    }
+    *addr = g_noalloc_addr[dev];
+    return MDSM_OK;
+}
+
+template <typename T>
+int launch_detect_noalloc_t(const T *series, int nbeams, int ndms, long long nsamps, long long n, double thr, mdsm_event *ev,
+                            long long max_events, unsigned long long *count, double *stats, cudaStream_t st)
+{
+    // Nothing in `stats` needs clearing: series_stats_kernel writes the pair of every (beam, dm) of this call before
+    // threshold_emit_kernel (same stream, so ordered after it) reads exactly those pairs.
+    series_stats_kernel<T><<<dim3(ndms, nbeams), kThreads, 0, st>>>(series, 0, ndms, nsamps, n, stats);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    dim3 g2((unsigned)((n + kThreads * 4 - 1) / (kThreads * 4)), ndms, nbeams);
+    threshold_emit_kernel<T><<<g2, kThreads, 0, st>>>(series, 0, ndms, nsamps, n, stats, thr, ev, max_events, count);
+    MDSM_CUDA_TRY(cudaGetLastError());
+    return MDSM_OK;
+}
+
+}  // namespace
+
+extern "C" int mdsm_detect_noalloc(const void *d_series, int dtype, int nbeams, int ndms, int64_t nsamps, int64_t nsamps_out,
+                                   double snr_thresh, mdsm_event *d_events, int64_t max_events, unsigned long long *d_count,
+                                   void *cuda_stream)
+{
+    MDSM_REQUIRE(d_series && d_count, "mdsm_detect_noalloc: null series or count pointer");
+    MDSM_REQUIRE(dtype == MDSM_F32 || dtype == MDSM_U8, "mdsm_detect_noalloc: dtype must be MDSM_F32 (float series) or MDSM_U8 (uint32 series)");
+    MDSM_REQUIRE(nbeams >= 1 && ndms >= 1 && nbeams <= 65535 && ndms <= 65535, "mdsm_detect_noalloc: nbeams and ndms must be in 1..65535");
+    MDSM_REQUIRE(nsamps_out >= 1 && nsamps_out <= nsamps, "mdsm_detect_noalloc: need 1 <= nsamps_out <= nsamps");
+    MDSM_REQUIRE((nsamps_out + kThreads * 4 - 1) / (kThreads * 4) <= 2147483647LL, "mdsm_detect_noalloc: series too long");
+    MDSM_REQUIRE(max_events >= 0 && (d_events || max_events == 0), "mdsm_detect_noalloc: bad event buffer");
+    MDSM_REQUIRE(snr_thresh == snr_thresh, "mdsm_detect_noalloc: snr_thresh must not be NaN");
+    MDSM_REQUIRE((long long)nbeams * ndms <= (long long)MDSM_DETECT_NOALLOC_MAX_SERIES,
+                 "mdsm_detect_noalloc: %lld series (nbeams * ndms) exceed the fixed scratch of MDSM_DETECT_NOALLOC_MAX_SERIES = %d series; "
+                 "this entry point never allocates, so split the series over several calls on one stream",
+                 (long long)nbeams * ndms, (int)MDSM_DETECT_NOALLOC_MAX_SERIES);
+    double *stats = nullptr;
+    const int rc = noalloc_scratch(&stats);
+    if (rc) return rc;
+    const cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (dtype == MDSM_F32)
+        return launch_detect_noalloc_t<float>((const float *)d_series, nbeams, ndms, nsamps, nsamps_out, snr_thresh, d_events,
+                                              max_events, d_count, stats, st);
+    return launch_detect_noalloc_t<uint32_t>((const uint32_t *)d_series, nbeams, ndms, nsamps, nsamps_out, snr_thresh, d_events,
+                                             max_events, d_count, stats, st);
+}

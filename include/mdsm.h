@@ -65,7 +65,8 @@ int64_t mdsm_plan_nsamps_out(const mdsm_plan *plan);                /* nsamps - 
 int mdsm_plan_get_delays(const mdsm_plan *plan, int32_t *h_delays);
 const char *mdsm_last_error(void);
 
-/* Plan options (synchronise the device; not for use while work of this plan is in flight).
+/* Plan options (not for use while work of this plan is in flight; "group_size" synchronises the device, the others
+ * only set a field).
  *  "dedisp_kernel": 0 = auto (the pre-summed-rows kernel whenever the plan has tables for it, else the direct kernel),
  *      1 = direct (one thread per output, global loads: the cross-check kernel), 2 = pre-summed rows or MDSM_EINVAL,
  *      3 = pre-summed rows with the operand windows staged in tensor memory (fp32 only; an experimental variant of the
@@ -74,6 +75,8 @@ const char *mdsm_last_error(void);
  *      rebuilds the tables and DROPS the scratch reservation (call mdsm_plan_reserve again).
  *  "detect_two_pass": 0 (default) = mdsm_detect is ONE launch (a CTA per series: statistics from HBM, thresholding of the same row
  *      out of L2); 1 = the two-launch form (statistics kernel, then a grid over (time, series)), kept for comparison.
+ *      Series too long for the one-launch kernel's shared memory (nsamps_out above about 5.2 million) take the two-launch form
+ *      by themselves.
  *  "post_median_window" (0 = off, else odd <= 33) and "post_detrend" (0/1): mdsm_pipeline_host runs
  *      mdsm_median_filter / mdsm_detrend on the fp32 series between dedispersion and detection (ignored for uint8).
  * Unknown key/value -> MDSM_EINVAL. */
@@ -81,15 +84,18 @@ int mdsm_plan_set_option(mdsm_plan *plan, const char *key, int64_t value);
 /* Allocates the plan-owned scratch of mdsm_dedisperse for `dtype`: the pre-summed channel-group rows (uint8: exact; fp32: same terms, another order)
  * (DESIGN.md section 6.1), nyrows * nsamps * (4 | 2) bytes per beam.  Call once after mdsm_plan_create (and after
  * changing "group_size") and before the first mdsm_dedisperse of that dtype; mdsm_pipeline_host calls it itself.
- * max_bytes = 0: as many beams as fit a quarter of the free device memory; otherwise at most max_bytes (never less
- * than one beam).  When the scratch holds fewer beams than the plan (mdsm_plan_kernel_info: scratch_slots < nbeams),
+ * max_bytes = 0: keep the reservation this dtype already has, whatever its size (so the call is a no-op once reserved, and
+ * a cap set earlier survives mdsm_pipeline_host's own call); with none yet, as many beams as fit a quarter of the free
+ * device memory.  max_bytes > 0: at most max_bytes (never less than one beam), replacing a reservation of another size.  When the scratch holds fewer beams than the plan (mdsm_plan_kernel_info: scratch_slots < nbeams),
  * mdsm_dedisperse walks its beams through it in stream order and calls for different beam ranges must then be issued
  * on ONE stream.  Synchronises the device only when an existing reservation has to be replaced.
  * Returns MDSM_ENOMEM if not even one beam fits. */
 int mdsm_plan_reserve(mdsm_plan *plan, int dtype, int64_t max_bytes);
 /* Which dedispersion kernel mdsm_dedisperse runs for `dtype` and with what geometry: writes a NUL-terminated list of
  * "key=value" words to buf ("kernel=rows group_size=4 ... scratch_slots=8 scratch_bytes=..." or
- * "kernel=direct reason=option|no_tables").  Returns 1 (rows), 0 (direct) or a negative MDSM_* status. */
+ * "kernel=direct reason=option|no_tables").  Returns 1 (rows), 0 (direct) or a negative MDSM_* status; with option
+ * dedisp_kernel = 3 and a dtype / plan the TMEM variant has no tables for it writes "kernel=none reason=tmem_f32_only|
+ * no_tmem_tables" and returns MDSM_EINVAL, as mdsm_dedisperse would. */
 int mdsm_plan_kernel_info(const mdsm_plan *plan, int dtype, char *buf, int64_t buflen);
 /* Number of kernels this plan has launched since creation (all entry points). */
 int64_t mdsm_plan_launch_count(const mdsm_plan *plan);

@@ -194,7 +194,7 @@ def mdsm_plan_kernel_info(plan, dtype: int) -> dict:
     """The C call's "key=value ..." description as a dict (integers where they parse)."""
     buf = ctypes.create_string_buffer(512)
     rc = _L.mdsm_plan_kernel_info(plan, dtype, buf, len(buf))
-    if rc < 0:
+    if rc < 0 and not buf.value:                     # "kernel=none reason=..." comes with MDSM_EINVAL and is still a description
         raise MdsmError(rc, mdsm_last_error())
     info = {}
     for kv in buf.value.decode().split():

@@ -1124,6 +1124,20 @@ static double group_cost(const mdsm_plan *p, const GroupRows &gr, bool packed16)
     return (double)p->ndms * gr.ngroups + (packed16 ? 16.0 : 11.0) * gr.nyrows;
 }
 
+// Dynamic shared memory of the pre-pass (group_presum_*): G rows of chunk + dmax samples in the input's element type, then
+// the group's pattern table.  kind 0: 32-bit samples (MDSM_F32, MDSM_U16), 1: uint8, 2: 4-bit.  delta_off = where the
+// pattern table starts.  Used at plan time (a group size that does not fit is skipped) and at launch time.
+constexpr size_t kPreSmemLimit = 200 * 1024;
+static size_t presum_smem_bytes(int kind, int G, int dmax, int maxpat, size_t *delta_off)
+{
+    const int chunk = kind == 0 ? kPreChunkF32 : kPreChunkU8;
+    const size_t rows = kind == 0 ? (size_t)G * (chunk + dmax) * 4
+                                  : (kind == 1 ? (size_t)G * (chunk + ((dmax + 3) & ~3) + 4) : (size_t)G * ((((chunk + dmax) / 2 + 3) & ~3) + 8));
+    const size_t off = (rows + 15) & ~(size_t)15;
+    if (delta_off) *delta_off = off;
+    return off + (size_t)maxpat * kGMax * sizeof(int16_t);
+}
+
 static int build_dtype(mdsm_plan *p, int kind /* 0: 32-bit rows, 1: uint8 -> 16-bit rows, 2: 4-bit -> 16-bit rows */, const std::vector<GroupRows> &cands)
 {
     const bool f32 = kind == 0;
@@ -1138,6 +1152,9 @@ static int build_dtype(mdsm_plan *p, int kind /* 0: 32-bit rows, 1: uint8 -> 16-
     for (const GroupRows *gr : order) {
         RowsHost h;
         if (!build_rows_tables(p, f32, kind == 2 ? kPartChansU4 : kPartChansU8, *gr, geom, rt, h)) continue;
+        // the pre-pass of this group size must fit its shared memory too, or every mdsm_dedisperse would fail at launch
+        // although kernel_info says "rows": try the next candidate (a smaller G has a smaller delay range per group)
+        if (presum_smem_bytes(kind, rt.G, rt.dmax, rt.maxpat, nullptr) > kPreSmemLimit) { rt = RowsTables(); continue; }
         if (!upload((int4 **)&rt.d_rowdesc, h.rowdesc) || !upload(&rt.d_ent, h.ent) || !upload(&rt.d_sigma, h.sigma) ||
             !upload(&rt.d_group_row0, gr->group_row0) || !upload(&rt.d_ydelta, gr->ydelta)) {
             mdsm_set_error("dedispersion table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -1234,11 +1251,9 @@ int mdsm_launch_dedisperse_rows(mdsm_plan *p, const void *d_in, int dtype, int b
     MDSM_REQUIRE(rt.ok && scratch && nslots >= 1, "dedispersion scratch not reserved (call mdsm_plan_reserve)");
     const int ntile_t = (int)((p->nsamps_out + rt.sigma_max + rt.stride - 1) / rt.stride);
     const int chunk = w32 ? kPreChunkF32 : kPreChunkU8;
-    const size_t pre_smem = w32 ? (size_t)rt.G * (chunk + rt.dmax) * 4
-                                : (dtype == MDSM_U8 ? (size_t)rt.G * (chunk + ((rt.dmax + 3) & ~3) + 4) : (size_t)rt.G * ((((chunk + rt.dmax) / 2 + 3) & ~3) + 8));
-    const size_t delta_off = (pre_smem + 15) & ~(size_t)15;
-    const size_t pre_smem_all = delta_off + (size_t)rt.maxpat * kGMax * sizeof(int16_t);
-    MDSM_REQUIRE(pre_smem_all <= 200 * 1024, "pre-pass: group delay range or pattern count too large");
+    size_t delta_off = 0;
+    const size_t pre_smem_all = presum_smem_bytes(w32 ? 0 : (dtype == MDSM_U8 ? 1 : 2), rt.G, rt.dmax, rt.maxpat, &delta_off);
+    MDSM_REQUIRE(pre_smem_all <= kPreSmemLimit, "pre-pass: group delay range or pattern count too large");   // plan time excludes it
     // beams go through the scratch `nslots` at a time (slot = beam % nslots), in stream order
     for (int bs = beam0; bs < beam0 + nb; bs += nslots) {
         const int n = std::min(nslots, beam0 + nb - bs);

@@ -277,8 +277,10 @@ int launch_detect_t(mdsm_plan *p, const T *out, int beam0, int nb, double thr, m
 {
     MDSM_REQUIRE(p->ndms <= 65535 && nb <= 65535, "ndms and nb must be <= 65535");
     dim3 g1(p->ndms, nb);
-    if (p->detect_two_pass) {
-        // the two-launch form (statistics, then a grid over (time, series)): kept for comparison (option "detect_two_pass")
+    const size_t fsmem = (size_t)((p->nsamps_out / 4 + 31) / 32 + 1) * sizeof(T);
+    if (p->detect_two_pass || fsmem > 160 * 1024) {
+        // the two-launch form (statistics, then a grid over (time, series)): option "detect_two_pass" for comparison, and
+        // by itself for series whose chunk maxima do not fit the fused kernel's shared memory (nsamps_out above ~5.2 M)
         series_stats_kernel<T><<<g1, kThreads, 0, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats);
         MDSM_CUDA_TRY(cudaGetLastError());
         dim3 g2((unsigned)((p->nsamps_out + kThreads * 4 - 1) / (kThreads * 4)), p->ndms, nb);
@@ -288,8 +290,6 @@ int launch_detect_t(mdsm_plan *p, const T *out, int beam0, int nb, double thr, m
         p->launches += 2;
         return MDSM_OK;
     }
-    const size_t fsmem = (size_t)((p->nsamps_out / 4 + 31) / 32 + 1) * sizeof(T);
-    MDSM_REQUIRE(fsmem <= 160 * 1024, "series too long for the fused detection kernel (set option detect_two_pass)");
     if (fsmem > 48 * 1024) MDSM_CUDA_TRY(cudaFuncSetAttribute(detect_fused_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
     detect_fused_kernel<T><<<g1, kFusedThreads, fsmem, st>>>(out, beam0, p->ndms, p->nsamps, p->nsamps_out, p->d_series_stats, thr, ev,
                                                         max_events, count);

@@ -41,9 +41,11 @@ __device__ __forceinline__ unsigned code_of(float x, double xmax, double mu, dou
     const float vf = mu_f >= 1.0f ? 255.0f * (__log2f(1.0f + mu_f * __fdividef(x, xmax_f)) * inv_den_f)
                                   : 255.0f * (log1pf(mu_f * (x / xmax_f)) * inv_den_f);
     const float fr = vf - floorf(vf);
-    // guard band: 1e-3 for log1pf; 2.5e-4 for the hardware log2 with mu >= 1 (its error in vf is below 5e-5: 2 ulp of a
-    // result <= log2(1 + mu), scaled by 255 / log2(1 + mu))
-    if (fabsf(fr - 0.5f) >= (mu_f >= 1.0f ? 2.5e-4f : 1e-3f)) return (unsigned)floorf(vf + 0.5f);
+    // guard band: 1e-3 for log1pf; 5e-4 for the hardware log2 with mu >= 1.  Worst-case error of vf on that path, at mu = 1
+    // (where the scale 255 / log2(1 + mu) is largest): MUFU.LG2's 2^-22 absolute error x 255 = 6e-5, __fdividef's 2 ulp and
+    // the fp32 rounding of 1 + a another ~5e-5 after the same scaling, the two product roundings near vf = 255 3e-5:
+    // about 1.5e-4 in all, so 5e-4 leaves a factor three (a band of 2.5e-4 left less than two).
+    if (fabsf(fr - 0.5f) >= (mu_f >= 1.0f ? 5e-4f : 1e-3f)) return (unsigned)floorf(vf + 0.5f);
     const double v = 255.0 * (log1p(mu * ((double)x / xmax)) * inv_den);
     return (unsigned)floor(v + 0.5);
 }

@@ -265,6 +265,10 @@ extern "C" int mdsm_plan_reserve(mdsm_plan *p, int dtype, int64_t max_bytes)
     void *&scratch = p->d_scratch[dtype];
     int &slots = p->scratch_slots[dtype];
     size_t &bytes = p->scratch_bytes[dtype];
+    // max_bytes = 0 asks for "a reservation", not for a new size: an existing one (the caller's explicit cap included)
+    // stays as it is.  Without this, mdsm_pipeline_host's own reserve call replaced a caller's cap, and on a device where
+    // not every beam fits the size derived from the free memory changed from call to call (free / realloc every buffer).
+    if (scratch && max_bytes == 0) return MDSM_OK;
     size_t limit = (size_t)max_bytes;
     if (limit == 0) {
         size_t free_b = 0, total_b = 0;
@@ -302,6 +306,12 @@ extern "C" int mdsm_plan_kernel_info(const mdsm_plan *p, int dtype, char *buf, i
     if (!rows) {
         snprintf(buf, (size_t)buflen, "kernel=direct reason=%s", p->dedisp_kernel == 1 ? "option" : "no_tables");
         return 0;
+    }
+    if (p->dedisp_kernel == 3 && !(f32 && p->tmem_f32.ok)) {
+        // the same verdict mdsm_dedisperse gives: the TMEM variant exists for fp32 plans with TMEM tables only
+        snprintf(buf, (size_t)buflen, "kernel=none reason=%s", f32 ? "no_tmem_tables" : "tmem_f32_only");
+        mdsm_set_error("dedisp_kernel = 3 (TMEM variant) has no tables for this plan / dtype: mdsm_dedisperse will return MDSM_EINVAL");
+        return MDSM_EINVAL;
     }
     const bool tmem = f32 && p->tmem_f32.ok && p->dedisp_kernel == 3;
     const TmemTables &tt = p->tmem_f32;

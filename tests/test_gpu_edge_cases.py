@@ -243,6 +243,13 @@ def test_scratch_smaller_than_the_plan_walks_the_beams_through_it(dtype):
         h_ev = np.zeros(1 << 16, dtype=m.EVENT_DTYPE)
         rc, cnt = m.mdsm_pipeline_host(p.h, x, 0, 0.0, 0.0, 4.0, h_ev, 1 << 16, 4)
         assert rc == m.MDSM_OK and abs(cnt - cnt_o) <= (0 if dtype == np.uint8 else 3)
+        # the pipeline's own mdsm_plan_reserve(plan, dtype, 0) must keep the caller's two-slot cap: only then did the call
+        # above take the one-stream branch this test is about
+        assert p.info(mdt)["scratch_slots"] == 2
+        m.mdsm_plan_reserve(p.h, mdt, 0)
+        assert p.info(mdt)["scratch_slots"] == 2
+        m.mdsm_plan_reserve(p.h, mdt, 3 * per_beam + 100)                  # an explicit size still replaces it
+        assert p.info(mdt)["scratch_slots"] == 3
 
 
 @pytest.mark.parametrize("G", [1, 2, 3, 4, 5, 6, 7, 8])
@@ -277,3 +284,34 @@ def test_kernel_info_reports_the_direct_kernel_and_its_reason():
         p.set_option("dedisp_kernel", 1)
         info = p.info(m.MDSM_U8)
         assert info["kernel"] == "direct" and info["reason"] == "option"
+        # option 3 (TMEM operands) exists for fp32 only: kernel_info and mdsm_dedisperse must give the same verdict
+        torch = _torch()
+        p.set_option("dedisp_kernel", 3)
+        info = p.info(m.MDSM_U8)
+        assert info["kernel"] == "none" and info["reason"] == "tmem_f32_only"
+        m.mdsm_plan_reserve(p.h, m.MDSM_U8, 0)
+        x = torch.zeros((1, 64, 4096), dtype=torch.uint8, device="cuda")
+        out = torch.zeros((1, 32, 4096), dtype=torch.int32, device="cuda")
+        with pytest.raises(m.MdsmError) as ei:
+            m.mdsm_dedisperse(p.h, x, 0, 1, out)
+        assert ei.value.status == m.MDSM_EINVAL
+
+
+def test_detect_on_a_series_too_long_for_the_one_launch_kernel_falls_back_by_itself():
+    """The fused detection kernel keeps one maximum per 128 samples in shared memory; beyond ~5.2 M samples that no longer
+    fits and mdsm_detect must take the two-launch form on its own (it used to return MDSM_EINVAL).  uint32: bit-exact."""
+    torch = _torch()
+    import paper_1307_5700_b200 as m
+    ns = 6_000_000
+    args = (1, 8, 418.0, -2.5, 51.2e-6, ns, 0.0, 0.15, 2)
+    g = np.random.default_rng(77)
+    with Plan(args) as p:
+        n = p.nsamps_out
+        s = (g.integers(0, 64, size=(1, 2, ns)) + 4000).astype(np.uint32)
+        s[0, 1, n - 1] += 700
+        s[0, 0, 5_500_000] += 900
+        ev_o, cnt_o, _ = oracle.detect(s, n, 6.0)
+        l0 = m.mdsm_plan_launch_count(p.h)
+        ev_g, cnt_g = p.detect(torch.from_numpy(s.view(np.int32)).cuda(), 6.0)
+        assert m.mdsm_plan_launch_count(p.h) - l0 == 2
+        assert cnt_g == cnt_o >= 2 and np.array_equal(ev_g, ev_o)

@@ -88,3 +88,36 @@ def test_random_plan_u8_chain_bit_exact(seed):
         hev = hev[:cnt]
         hev = hev[np.lexsort((hev["t"], hev["dm_idx"], hev["beam"]))]
         assert np.array_equal(hev, ev_o), args
+
+
+@pytest.mark.parametrize("G", [0, 8, 3])
+def test_wide_sweep_at_low_frequency_picks_a_group_size_whose_pre_pass_fits(G):
+    """A low band with a large DM: adjacent channels are thousands of samples apart, so the pre-pass of a wide channel
+    group (G rows of chunk + delay range samples in shared memory) does not fit.  The plan must skip such a group size
+    when it builds its tables -- or report the direct kernel for an explicit one -- instead of reporting kernel=rows and then
+    failing every mdsm_dedisperse call at launch.  Whatever it picks has to run in 'auto' mode and match the oracle."""
+    import torch
+    import paper_1307_5700_b200 as m
+    nchans, f_top, foff, tsamp, dm_low, dm_step, ndms = 48, 60.0, -0.25, 51.2e-6, 0.0, 0.7, 12
+    d = oracle.delay_table(nchans, f_top, foff, tsamp, dm_low, dm_step, ndms)
+    assert int(np.diff(d[-1]).max()) > 2000                     # adjacent channels, last DM: thousands of samples
+    ns = int(d.max()) + 5000
+    ns += (-ns) % 16
+    args = (1, nchans, f_top, foff, tsamp, ns, dm_low, dm_step, ndms)
+    g = np.random.default_rng(7)
+    xf = (g.normal(size=(1, nchans, ns)) + 3.0).astype(np.float32)
+    xu = g.integers(0, 256, size=(1, nchans, ns)).astype(np.uint8)
+    with Plan(args) as p:
+        if G:
+            p.set_option("group_size", G)
+        for x, mdt in ((xf, m.MDSM_F32), (xu, m.MDSM_U8)):
+            info = p.info(mdt)
+            assert info["kernel"] in ("rows", "direct"), info
+            if G == 8 and mdt == m.MDSM_F32:                    # 8 rows x (2048 + ~18000) words = 640 KB (bytes still fit: 177 KB)
+                assert info["kernel"] == "direct" and info["reason"] == "no_tables", info
+            ref, ab = oracle.dedisperse(x, d)
+            got = out_to_numpy(p.dedisperse(torch.from_numpy(x).cuda(), kernel=0), p.nsamps_out)
+            if mdt == m.MDSM_U8:
+                assert np.array_equal(got, ref), info
+            else:
+                assert np.all(np.abs(got.astype(np.float64) - ref) <= 1e-5 * ab + 1e-6), info

@@ -65,6 +65,20 @@ def test_band_edge_channel_takes_its_only_clean_neighbour():
     assert r["nmasked"][0] == 1 and r["bpi"][0, 0] == 2.0 and np.allclose(r["fit"][0], 2.0, atol=1e-14)
 
 
+def test_mask_limit_is_k_times_1_4826_mad_pinned_from_both_sides():
+    """Reading H-ii: a channel is masked when bp - median > k_mask * 1.4826 * MAD.  bp = 1..9: median 5, deviations
+    4,3,2,1,0,1,2,3,4, MAD 2, so the limit is 2.9652 * k_mask.  Channel 8 (bp = 9, 4 above the median) sits exactly on the
+    limit at k_mask = 4 / 2.9652 = 1.34898...: k = 1.3489 masks it (limit 3.99976), k = 1.3491 does not (4.00035), which
+    pins the constant to 1.4826 +- 0.0001; k = 1.3 masks channel 8 only, where a limit of k * MAD (no 1.4826: 2.6) would
+    also take channel 7 (3 above), and k * 1.4826 * std (std = 2.582: 4.98) would take none."""
+    bp = np.arange(1.0, 10.0)
+    x = np.repeat(bp[None, :, None], 64, axis=2).astype(np.float32)
+    for k_mask, masked in ((1.3489, [8]), (1.3491, []), (1.3, [8]), (1.0, [7, 8]), (0.68, [7, 8]), (0.67, [6, 7, 8])):
+        r = oracle.bandpass_clip(x.copy(), 8, 0, k_mask, 1e9, 1e9, subtract=False)
+        got = np.flatnonzero(r["bpi"][0] != bp).tolist()
+        assert r["nmasked"][0] == len(masked) and got == masked, (k_mask, got)
+
+
 def test_constant_input_order0_no_flags_strict_comparison():
     x = np.full((2, 8, 256), 3.0, dtype=np.float32)
     r = oracle.bandpass_clip(x, 32, 0, 5.0, 0.0, 0.0, subtract=False)     # k = 0: thresholds sit exactly on the data
@@ -173,6 +187,52 @@ def test_fdbscan_equals_dbscan_on_compact_separated_blobs():
     lab, ncl = oracle.dbscan(pts, [8.0, 2.0, 1.5], 4)
     labf, nclf, nq = oracle.fdbscan(pts, [8.0, 2.0, 1.5], 4)
     assert ncl == nclf == 3 and np.array_equal(lab, labf)
+
+
+def _pins():
+    import os
+    import runpy
+    return runpy.run_path(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "fdbscan_pins.py"))
+
+
+@pytest.mark.parametrize("name", ["split", "lost", "other"])
+def test_fdbscan_hand_worked_sets_labels_and_query_counts(name):
+    """PAPER.md:126, reading K-ii.  Expected labels and query counts are written out by hand in tests/golden/fdbscan_pins.py
+    (walk-through above each set), not produced by the oracle.  Each set fails for one plausible one-line misreading, and this
+    was checked by applying the mutation to oracle/mdsm_oracle_next.c (orc_fdbscan) and re-running this test:
+      split -- `v > bestv` turned into "nearest" (smallest positive v): labels become one cluster;
+      lost  -- `v > bestv` -> `v >= bestv` (ties to the higher index): points 3 and 4 join the cluster;
+      other -- the `label[r] != cid` filter removed (representatives among all neighbours): point 8 becomes noise.
+    The DBSCAN labels of the same sets are pinned by scikit-learn, so "split" exhibits the paper's "clusters might be split
+    apart" and "lost" its "some points might be lost" against an independent exact clustering."""
+    sk = pytest.importorskip("sklearn.cluster")
+    S = _pins()["SETS"][name]
+    pts = np.array([(t, d, 10.0) for t, d in S["pts"]], dtype=np.float64)
+    eps = np.array([S["eps"], S["eps"], 1.0])
+    lab, ncl, nq = oracle.fdbscan(pts, eps, S["min_pts"])
+    assert lab.tolist() == S["fdbscan_labels"], S["fails_for"]
+    assert ncl == max(S["fdbscan_labels"]) + 1 and nq == S["fdbscan_queries"], S["fails_for"]
+    ref = sk.DBSCAN(eps=1.0, min_samples=S["min_pts"], metric="chebyshev").fit(pts / eps)
+    assert ref.labels_.tolist() == S["dbscan_labels"]
+    assert oracle.dbscan(pts, eps, S["min_pts"])[0].tolist() == S["dbscan_labels"]
+    # the same set with the second coordinate in the SNR dimension instead of DM: dimension 2 is treated like the others
+    pts3 = np.array([(t, 3.0, d) for t, d in S["pts"]], dtype=np.float64)
+    lab3, _, nq3 = oracle.fdbscan(pts3, np.array([S["eps"], 1.0, S["eps"]]), S["min_pts"])
+    assert lab3.tolist() == S["fdbscan_labels"] and nq3 == S["fdbscan_queries"]
+
+
+@pytest.mark.parametrize("dim", [0, 1, 2])
+@pytest.mark.parametrize("sign", [1, -1])
+def test_fdbscan_chain_along_every_dimension_and_direction(dim, sign):
+    """"Two for each dimension, one for each direction": a row of points along one axis is followed to its
+    end through the far representative only (4 queries for 7 points; the nearest-representative misreading needs 7, a
+    dimension or direction left out breaks the row into several clusters)."""
+    C = _pins()["CHAIN"]
+    pts = np.zeros((C["n"], 3))
+    pts[:, 2] = 10.0
+    pts[:, dim] += sign * C["step"] * np.arange(C["n"])
+    lab, ncl, nq = oracle.fdbscan(pts, [C["eps"]] * 3, C["min_pts"])
+    assert ncl == 1 and lab.tolist() == [0] * C["n"] and nq == C["fdbscan_queries"], C["fails_for"]
 
 
 # ------------------------------------------------------------------ classifier (Eqs. 3, 4)

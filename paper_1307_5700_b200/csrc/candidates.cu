@@ -1,7 +1,8 @@
 // Host candidate stage (BASELINE.json north_star: "DBSCAN-style clustering and the analytic DM-SNR
 // candidate filter stay on the host"): FDBSCAN over the (time, DM, SNR) detections and the eight-step
-// DM-SNR-curve classifier with Eqs. 3 and 4.  Plain host C++ (no device work); region queries go
-// through a uniform grid of eps-sized cells instead of the O(N^2) scan of the oracle.
+// DM-SNR-curve classifier with Eqs. 3 and 4.  Plain host C++ (no device work).  Region queries go
+// through a uniform grid of eps-sized cells; the six FDBSCAN representatives come out of one sweep over a neighbour
+// list; the classifier works on a DM-sorted event list reduced to one row per DM trial.
 #include <algorithm>
 #include <cmath>
 #include <unordered_map>
@@ -55,78 +56,157 @@ struct Grid {
     }
 };
 
-constexpr int32_t kUnclassified = -2, kNoise = -1;
+// ---- density clustering of one beam's detections ------------------------------------------------------------------
+// PAPER.md:118-126.  A cluster is grown from a core point ("seed") through a FIFO of points still to be examined.
+// DBSCAN (exact): every member found goes through the FIFO.  FDBSCAN: of a core point's neighbourhood only
+// the six border representatives do -- "two for each dimension, one for each direction when placing the core point at
+// the origin" -- found in ONE sweep over the neighbour list that keeps, per (dimension, direction) slot, the member of the
+// growing cluster with the largest displacement (strictly positive; neighbour lists are ascending, so the first of
+// equally far points stays).  Neighbour lists come from the grid above.
+class BeamClusterer {
+public:
+    BeamClusterer(const std::vector<Point> &pts, const double *eps, int min_pts, int32_t *label)
+        : pts_(pts), grid_(pts, eps), min_pts_(min_pts), label_(label), in_fifo_(pts.size(), 0)
+    {
+        std::fill(label_, label_ + pts.size(), kFresh);
+    }
 
-// One beam's detections, points in the caller's order.  exact = 1: DBSCAN (every neighbour of a core point is expanded);
-// exact = 0: FDBSCAN: only the representative border points of a core point's neighbourhood -- per
-// dimension and direction the neighbour of this cluster farthest from the core point, the lowest index among equals --
-// are expanded, each point at most once.
-int64_t cluster_beam(const std::vector<Point> &pts, const double *eps, int min_pts, bool exact, int32_t *label, int32_t first_id,
-                     int64_t *n_queries)
-{
-    const int32_t n = (int32_t)pts.size();
-    Grid grid(pts, eps);
-    std::vector<int32_t> nb, queue;
-    std::vector<uint8_t> done(n, 0);            // DBSCAN: queued; FDBSCAN: expanded
-    for (int32_t i = 0; i < n; ++i) label[i] = kUnclassified;
-    int32_t cid = first_id;
-    for (int32_t p = 0; p < n; ++p) {
-        if (label[p] != kUnclassified) continue;
-        grid.query(p, nb);
-        ++*n_queries;
-        if ((int)nb.size() < min_pts) { label[p] = kNoise; continue; }
-        queue.clear();
-        size_t head = 0;
-        if (exact) {
-            label[p] = cid;
-            queue.push_back(p);
-            done[p] = 1;
-            while (head < queue.size()) {
-                const int32_t q = queue[head++];
-                grid.query(q, nb);
-                ++*n_queries;
-                if ((int)nb.size() < min_pts) continue;
-                for (int32_t r : nb) {
-                    if (label[r] == kUnclassified || label[r] == kNoise) label[r] = cid;
-                    if (label[r] == cid && !done[r]) { queue.push_back(r); done[r] = 1; }
-                }
-            }
-        } else {
-            queue.push_back(p);
-            bool first = true;
-            while (head < queue.size()) {
-                const int32_t q = queue[head++];
-                if (done[q]) continue;
-                done[q] = 1;
-                if (!first) { grid.query(q, nb); ++*n_queries; }
-                first = false;
-                if ((int)nb.size() < min_pts) continue;
-                for (int32_t r : nb)
-                    if (label[r] == kUnclassified || label[r] == kNoise) label[r] = cid;
-                for (int dim = 0; dim < 3; ++dim)
-                    for (int dir = 1; dir >= -1; dir -= 2) {
-                        int32_t best = -1;
-                        double bestv = 0.0;
-                        for (int32_t r : nb) {
-                            if (label[r] != cid) continue;
-                            const double v = (double)dir * (pts[r].x[dim] - pts[q].x[dim]);
-                            if (v > bestv) { bestv = v; best = r; }
-                        }
-                        if (best >= 0 && !done[best]) queue.push_back(best);
-                    }
+    // Returns the number of clusters found; ids start at first_id.
+    int64_t run(bool exact, int32_t first_id)
+    {
+        int32_t next_id = first_id;
+        for (int32_t p = 0; p < (int32_t)pts_.size(); ++p) {
+            if (label_[p] != kFresh) continue;
+            if (!core_neighbourhood(p)) { label_[p] = kNoiseLabel; continue; }
+            cid_ = next_id++;
+            fifo_.clear();
+            in_fifo_[p] = 1;                                   // the seed is being examined right now, with nb_ in hand
+            absorb(exact);
+            for (size_t head = 0; head < fifo_.size(); ++head)
+                if (core_neighbourhood(fifo_[head])) { centre_ = fifo_[head]; absorb(exact); }
+        }
+        return next_id - first_id;
+    }
+    int64_t queries() const { return queries_; }
+
+private:
+    static constexpr int32_t kFresh = -2, kNoiseLabel = -1;
+
+    // Region query around p into nb_; true when p is a core point.  Sets centre_.
+    bool core_neighbourhood(int32_t p)
+    {
+        centre_ = p;
+        grid_.query(p, nb_);
+        ++queries_;
+        return (int)nb_.size() >= min_pts_;
+    }
+
+    void enqueue(int32_t r)
+    {
+        if (in_fifo_[r]) return;                               // examined, or waiting to be: a point is examined once
+        in_fifo_[r] = 1;
+        fifo_.push_back(r);
+    }
+
+    // nb_ is the neighbourhood of the core point centre_: its unclaimed points (fresh or noise) join the cluster, then the
+    // points to examine next are queued: all members (DBSCAN) or the six representatives (FDBSCAN).
+    void absorb(bool exact)
+    {
+        int32_t far[6] = {-1, -1, -1, -1, -1, -1};             // slot 2 * dim + (0: towards larger, 1: towards smaller values)
+        double reach[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        const Point &c = pts_[centre_];
+        for (int32_t r : nb_) {
+            if (label_[r] < 0) label_[r] = cid_;
+            if (label_[r] != cid_) continue;                   // a border point another cluster claimed first stays there
+            if (exact) { enqueue(r); continue; }
+            for (int dim = 0; dim < 3; ++dim) {
+                const double off = pts_[r].x[dim] - c.x[dim];
+                const int slot = 2 * dim + (off < 0.0 ? 1 : 0);
+                if (std::fabs(off) > reach[slot]) { reach[slot] = std::fabs(off); far[slot] = r; }
             }
         }
-        ++cid;
+        if (!exact)
+            for (int slot = 0; slot < 6; ++slot)
+                if (far[slot] >= 0) enqueue(far[slot]);
     }
-    return cid - first_id;
-}
 
-// Eq. 3 with Eq. 4
-double dm_curve(double ddm, double bw_mhz, double w_ms, double nu_ghz)
+    const std::vector<Point> &pts_;
+    Grid grid_;
+    int min_pts_;
+    int32_t *label_;
+    std::vector<uint8_t> in_fifo_;
+    std::vector<int32_t> nb_, fifo_;
+    int32_t centre_ = 0, cid_ = 0;
+    int64_t queries_ = 0;
+};
+
+// ---- DM-SNR classifier ---------------------------------------------------------------------------------------------
+// Eq. 3 at the zeta of Eq. 4: the fraction of a pulse's peak that survives dedispersion at a
+// DM that is ddm off, for a pulse of width w_ms observed over bw_mhz at nu_ghz.
+double surviving_fraction(double ddm, double bw_mhz, double w_ms, double nu_ghz)
 {
     const double zeta = std::fabs(6.91e-3 * ddm * bw_mhz / (w_ms * (nu_ghz * nu_ghz * nu_ghz)));
-    if (zeta < 1e-12) return 1.0;
-    return 0.5 * std::sqrt(3.14159265358979323846) * std::erf(zeta) / zeta;
+    return zeta < 1e-12 ? 1.0 : 0.5 * std::sqrt(3.14159265358979323846) * std::erf(zeta) / zeta;
+}
+
+// What the detections of one cluster at one DM trial collapse to (PAPER.md:146 step 1: "collapsing the time dimension").
+struct DmRow {
+    int32_t dm_idx;
+    int64_t count;        // detections at this DM
+    double peak;          // the strongest of them
+    int32_t t_first, t_last;
+};
+
+// Steps 1-8 of PAPER.md:144-156 for one cluster; `order` lists its events sorted by DM index.
+void classify_one(const mdsm_event *ev, const int64_t *order, int64_t m, double dm_low, double dm_step, double tsamp, double bw_mhz,
+                  double nu_ghz, int k_smooth, double rmse_max, std::vector<DmRow> &rows, std::vector<double> &sig, double *res)
+{
+    // 1: one sweep over the DM-sorted events gives a row per DM that has detections
+    rows.clear();
+    for (int64_t k = 0; k < m; ++k) {
+        const mdsm_event &e = ev[order[k]];
+        if (rows.empty() || rows.back().dm_idx != e.dm_idx) rows.push_back(DmRow{e.dm_idx, 0, (double)e.snr, e.t, e.t});
+        DmRow &r = rows.back();
+        r.count += 1;
+        r.peak = std::max(r.peak, (double)e.snr);
+        r.t_first = std::min(r.t_first, e.t);
+        r.t_last = std::max(r.t_last, e.t);
+    }
+    // 3, 4: the DM with the most detections (the lowest such DM), its strongest detection, the pulse width there
+    const DmRow *best = &rows[0];
+    for (const DmRow &r : rows)
+        if (r.count > best->count) best = &r;
+    const double dm_best = dm_low + (double)best->dm_idx * dm_step;
+    const double w_ms = (double)(best->t_last - best->t_first + 1) * tsamp * 1e3;
+    res[1] = (double)best->dm_idx; res[2] = best->peak; res[3] = w_ms;
+    if (dm_best < 1.0) { res[0] = 1.0; res[4] = 0.0; return; }           // broadband RFI (step 3)
+    // the signature on the dense DM axis of the cluster (0 where a DM trial has no detection)
+    const int32_t d_lo = rows.front().dm_idx;
+    const int nd = rows.back().dm_idx - d_lo + 1;
+    sig.assign((size_t)nd, 0.0);
+    for (const DmRow &r : rows) sig[(size_t)(r.dm_idx - d_lo)] = r.peak;
+    // 2, 5: centred k-element moving average (shorter at the two ends), then its maximum for the normalisation
+    const int half = k_smooth / 2;
+    std::vector<double> &smooth = sig;                                      // smoothed values are appended behind the raw ones
+    smooth.resize((size_t)2 * nd);
+    double top = 0.0;
+    for (int d = 0; d < nd; ++d) {
+        const int lo = std::max(0, d - half), hi = std::min(nd - 1, d + half);
+        double acc = 0.0;
+        for (int e = lo; e <= hi; ++e) acc += sig[(size_t)e];
+        smooth[(size_t)nd + d] = acc / (double)(hi - lo + 1);
+        top = std::max(top, smooth[(size_t)nd + d]);
+    }
+    // 6, 7: squared distance between the model curve around dm_best and the normalised signature
+    double sq = 0.0;
+    for (int d = 0; d < nd; ++d) {
+        const double ddm = (dm_low + (double)(d + d_lo) * dm_step) - dm_best;
+        const double shape = top > 0.0 ? smooth[(size_t)nd + d] / top : 0.0;
+        const double miss = surviving_fraction(ddm, bw_mhz, w_ms, nu_ghz) - shape;
+        sq += miss * miss;
+    }
+    res[4] = std::sqrt(sq / (double)nd);
+    res[0] = res[4] > rmse_max ? 2.0 : 0.0;                                  // 8
 }
 
 }  // namespace
@@ -160,7 +240,9 @@ extern "C" int mdsm_cluster_events(const mdsm_event *h_events, int64_t n, double
             pts[k].x[1] = dm_low + (double)e.dm_idx * dm_step;
             pts[k].x[2] = (double)e.snr;
         }
-        ncl += cluster_beam(pts, eps, min_pts, exact != 0, lab.data(), (int32_t)ncl, &nq);
+        BeamClusterer clusterer(pts, eps, min_pts, lab.data());
+        ncl += clusterer.run(exact != 0, (int32_t)ncl);
+        nq += clusterer.queries();
         for (size_t k = 0; k < idx.size(); ++k) h_labels[idx[k]] = lab[k];
     }
     *h_nclusters = ncl;
@@ -174,55 +256,28 @@ extern "C" int mdsm_classify_clusters(const mdsm_event *h_events, const int32_t 
 {
     MDSM_REQUIRE(n >= 0 && nclusters >= 0 && (n == 0 || (h_events && h_labels)) && (nclusters == 0 || h_results), "null argument");
     MDSM_REQUIRE(k_smooth >= 1 && (k_smooth & 1) && tsamp > 0.0 && bw_mhz > 0.0 && nu_ghz > 0.0, "k_smooth must be odd, tsamp, bandwidth and frequency > 0");
-    std::vector<std::vector<int64_t>> members((size_t)nclusters);
+    // group the events by cluster (counting sort on the label), then order each group by DM index
+    std::vector<int64_t> start((size_t)nclusters + 1, 0), order;
     for (int64_t i = 0; i < n; ++i) {
         MDSM_REQUIRE(h_labels[i] < nclusters, "label %d out of range", h_labels[i]);
-        if (h_labels[i] >= 0) members[(size_t)h_labels[i]].push_back(i);
+        if (h_labels[i] >= 0) ++start[(size_t)h_labels[i] + 1];
     }
-    std::vector<double> sig, sm;
-    std::vector<int64_t> cnt;
+    for (int64_t c = 0; c < nclusters; ++c) start[(size_t)c + 1] += start[(size_t)c];
+    order.resize((size_t)start[(size_t)nclusters]);
+    {
+        std::vector<int64_t> fill(start.begin(), start.end() - 1);
+        for (int64_t i = 0; i < n; ++i)
+            if (h_labels[i] >= 0) order[(size_t)fill[(size_t)h_labels[i]]++] = i;
+    }
+    std::vector<DmRow> rows;
+    std::vector<double> sig;
     for (int64_t c = 0; c < nclusters; ++c) {
         double *res = h_results + 5 * c;
-        const std::vector<int64_t> &m = members[(size_t)c];
-        if (m.empty()) { res[0] = -1.0; res[1] = res[2] = res[3] = res[4] = 0.0; continue; }
-        int dmin = h_events[m[0]].dm_idx, dmax = dmin;
-        for (int64_t i : m) { dmin = std::min(dmin, h_events[i].dm_idx); dmax = std::max(dmax, h_events[i].dm_idx); }
-        const int nd = dmax - dmin + 1;
-        sig.assign(nd, 0.0); sm.assign(nd, 0.0); cnt.assign(nd, 0);
-        for (int64_t i : m) {                                              // 1: collapse the time dimension
-            const int d = h_events[i].dm_idx - dmin;
-            if (cnt[d] == 0 || (double)h_events[i].snr > sig[d]) sig[d] = (double)h_events[i].snr;
-            ++cnt[d];
-        }
-        const int h = k_smooth / 2;                                        // 2: k-element moving average
-        for (int d = 0; d < nd; ++d) {
-            double s = 0.0; int k = 0;
-            for (int e = std::max(0, d - h); e <= std::min(nd - 1, d + h); ++e) { s += sig[e]; ++k; }
-            sm[d] = s / (double)k;
-        }
-        int dstar = 0;                                                     // 3: the DM with the most detections
-        for (int d = 1; d < nd; ++d) if (cnt[d] > cnt[dstar]) dstar = d;
-        const double dm_star = dm_low + (double)(dstar + dmin) * dm_step;
-        int32_t t0 = 0, t1 = 0; bool have = false;                         // 4: width at that DM
-        for (int64_t i : m)
-            if (h_events[i].dm_idx - dmin == dstar) {
-                if (!have || h_events[i].t < t0) t0 = h_events[i].t;
-                if (!have || h_events[i].t > t1) t1 = h_events[i].t;
-                have = true;
-            }
-        const double w_ms = (double)(t1 - t0 + 1) * tsamp * 1e3;
-        res[1] = (double)(dstar + dmin); res[2] = sig[dstar]; res[3] = w_ms;
-        if (dm_star < 1.0) { res[0] = 1.0; res[4] = 0.0; continue; }       //    DM < 1: broadband RFI
-        double mx = 0.0;                                                   // 5: normalise
-        for (int d = 0; d < nd; ++d) mx = std::max(mx, sm[d]);
-        double se = 0.0;                                                   // 6, 7: model curve and RMSE
-        for (int d = 0; d < nd; ++d) {
-            const double ddm = (dm_low + (double)(d + dmin) * dm_step) - dm_star;
-            const double e = dm_curve(ddm, bw_mhz, w_ms, nu_ghz) - (mx > 0.0 ? sm[d] / mx : 0.0);
-            se += e * e;
-        }
-        res[4] = std::sqrt(se / (double)nd);
-        res[0] = res[4] > rmse_max ? 2.0 : 0.0;                            // 8
+        int64_t *first = order.data() + start[(size_t)c];
+        const int64_t m = start[(size_t)c + 1] - start[(size_t)c];
+        if (m == 0) { res[0] = -1.0; res[1] = res[2] = res[3] = res[4] = 0.0; continue; }
+        std::stable_sort(first, first + m, [&](int64_t a, int64_t b) { return h_events[a].dm_idx < h_events[b].dm_idx; });
+        classify_one(h_events, first, m, dm_low, dm_step, tsamp, bw_mhz, nu_ghz, k_smooth, rmse_max, rows, sig, res);
     }
     return MDSM_OK;
 }

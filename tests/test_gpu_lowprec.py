@@ -56,6 +56,39 @@ def test_low_precision_inputs_bit_exact(name, kind, kernel):
         assert np.all(out[:, :, p.nsamps_out:].cpu().numpy() == -7)
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("kind", ["u16", "u4"])
+def test_low_precision_inputs_at_config_3_size_one_beam_every_element(kind):
+    """One beam of the configuration the headline metric is quoted on (1024 channels x 65536 samples, 640 DM trials, the
+    launch geometry bench.py times): every output element of the 16-bit and of the packed 4-bit input path against the oracle,
+    bit for bit.  Seeded noise with a saturated stretch and a dispersed pulse."""
+    import torch
+    from workloads import CONFIGS
+    cfg = CONFIGS[3]
+    args = (1,) + cfg.plan_args()[1:]
+    nc, ns, nd = cfg.nchans, cfg.nsamps, cfg.ndms
+    delay = oracle.delay_table(nc, cfg.f_top, cfg.foff, cfg.tsamp, cfg.dm_low, cfg.dm_step, nd)
+    g = np.random.default_rng(33)
+    top = 65535 if kind == "u16" else 15
+    v = g.integers(0, top + 1, size=(1, nc, ns), dtype=np.uint16)
+    v[:, :, 5000:5256] = top
+    v[0, np.arange(nc), 20000 + delay[333]] = top
+    ref = oracle.dedisperse_u16(v, delay)
+    d_in = torch.from_numpy(v.view(np.int16)).cuda() if kind == "u16" else torch.from_numpy(_pack_u4(v.astype(np.uint8))).cuda()
+    with Plan(args) as p:
+        m = p.m
+        dt = m.MDSM_U16 if kind == "u16" else m.MDSM_U4
+        m.mdsm_plan_reserve(p.h, dt, 0)
+        assert p.info(dt)["kernel"] == "rows"
+        out = torch.full((1, nd, ns), -7, dtype=torch.int32, device="cuda")
+        m.mdsm_dedisperse(p.h, d_in, 0, 1, out, dtype=dt)
+        torch.cuda.synchronize()
+        got = out[:, :, :p.nsamps_out].cpu().numpy().view(np.uint32)
+        assert np.array_equal(got, ref)
+        assert int(got[0, 333, 20000]) >= (nc - 1) * top // 2 + top          # the pulse adds up at its DM
+        assert np.all(out[:, :, p.nsamps_out:].cpu().numpy() == -7)
+
+
 def test_u4_4096_channels_one_part_and_odd_nsamps_refused():
     import torch
     args = (1, 4096, 418.0, -20.0 / 4096, 51.2e-6, 8192, 0.0, 0.5, 24)

@@ -24,6 +24,17 @@ _LIB = os.path.join(_HERE, "libmdsm_oracle.so")
 # -ffp-contract=off / no fast-math: every fp64 op is a single IEEE op in the order written.
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-Wall"]
 
+# MDSM_ORACLE_SANITIZE=1: the same sources with AddressSanitizer + UndefinedBehaviorSanitizer, in a library of its own
+# (SURVEY section 5).  An ASan library only loads into a process that has the ASan runtime first in line:
+#   MDSM_ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+#       python -m pytest tests -m "not gpu" -q
+# (leak detection off: CPython itself never frees everything).  Any finding aborts the process with a report.
+SANITIZE = os.environ.get("MDSM_ORACLE_SANITIZE", "0") not in ("", "0")
+if SANITIZE:
+    _LIB = os.path.join(_HERE, "libmdsm_oracle_san.so")
+    CFLAGS = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+              "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-Wall"]
+
 EVENT_DTYPE = np.dtype([("beam", "<i4"), ("dm_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
 
 

@@ -4,6 +4,10 @@
  *
  *   RFI clip  ->  multibeam brute-force incoherent dedispersion  ->  n-sigma detection
  *
+ * Call order of the hot path: mdsm_plan_create, mdsm_plan_reserve (once per sample type: the stage calls never allocate, so the
+ * dedispersion scratch is reserved up front -- mdsm_dedisperse returns MDSM_EINVAL without it), then per buffer mdsm_rfi_clip,
+ * mdsm_dedisperse, mdsm_detect; or mdsm_pipeline_host, which does all of it from host buffers.
+ *
  * Citations are to /root/reference/PAPER.md (line numbers) and to the readings listed in
  * DESIGN.md section 3.  All pointers named d_* are DEVICE pointers, h_* are HOST pointers.
  * The caller owns every buffer it passes; the plan owns the delay table and its scratch.
